@@ -1,0 +1,128 @@
+/* dg_habc.h — C ABI of the B200 nodal-DG + HABC time stepper (arXiv 1610.05023).
+ *
+ * One explicit LSRK4(5) time step of the nodal discontinuous Galerkin semi-discretisation of the acoustic
+ * pressure-velocity system (eq (1a-b)) on an affine tetrahedral mesh of a cuboid, with the
+ * multidimensional Padé high-order absorbing boundary condition on all six faces: 2D auxiliary solvers on
+ * the faces, 1D on the edges, 0D compatibility systems at the corners (Algorithm 1).
+ *
+ * Symbols follow BASELINE.json: N = polynomial degree (the paper's P), J = number of auxiliary fields per
+ * face (the paper's N), M = 2J+1.  Np = (N+1)(N+2)(N+3)/6, Nfp = (N+1)(N+2)/2 (Table 1).
+ *
+ * Conventions
+ *   - every pointer argument is a HOST pointer unless its name ends in _dev;
+ *   - interface arrays are float64, element-major [K][Np], in the library's node order (dg_get_nodes) and the
+ *     caller's element order; the device layout (node-major, field-interleaved, fp64 or fp32) is private;
+ *   - the library copies what it is given: the caller keeps ownership of every buffer it passes, and
+ *     outputs are written into caller-allocated buffers;
+ *   - every call returns DG_OK (0) or a negative DG_E* code; dg_last_error() returns the message of the
+ *     last failing call on this thread;
+ *   - all device work is enqueued on the stream given in dg_options (the CUDA stream handle, e.g.
+ *     torch.cuda.current_stream().cuda_stream); dg_step is asynchronous, the dg_get_* calls synchronise.
+ */
+#ifndef DG_HABC_H
+#define DG_HABC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DG_OK 0
+#define DG_EINVAL (-1) /* bad argument: N outside 1..8, J outside 0..12, NULL pointer, non-cuboid boundary */
+#define DG_EMESH (-2)  /* degenerate or non-conforming mesh */
+#define DG_ECUDA (-3)  /* CUDA runtime error (no device, launch failure, ...) */
+#define DG_ENOMEM (-4) /* workspace too small / allocation failed */
+
+typedef struct dg_solver dg_solver; /* opaque, owned by the library; free with dg_destroy */
+
+/* Tetrahedral mesh of a cuboid.  Any vertex order inside a tetrahedron is accepted
+ * (negatively oriented cells are re-oriented internally).  The six planes bounding the vertex cloud are the
+ * domain faces; all of them carry the HABC. */
+typedef struct {
+    int32_t nverts;
+    const double* xyz;   /* [nverts][3] */
+    int32_t ntets;
+    const int32_t* tets; /* [ntets][4] */
+} dg_mesh;
+
+typedef struct {
+    int32_t precision;        /* 64 or 32: arithmetic and storage type of the device state */
+    double cfl;               /* multiplies the time-step rule, eq (46) PAPER.md:L796 (reading R7); <=0 means 1.0 */
+    double dt;                /* > 0 overrides eq (46) */
+    void* stream;             /* cudaStream_t, or NULL for the default stream */
+    int32_t device;           /* CUDA device ordinal */
+    void* workspace_dev;      /* optional DEVICE buffer (e.g. torch-allocated) of workspace_bytes; NULL: cudaMalloc */
+    uint64_t workspace_bytes; /* size of workspace_dev; see dg_workspace_bytes */
+    int32_t use_graph;        /* 1: replay the 5-stage step as a CUDA graph; ignored (plain launches) when stream is NULL,
+                                 because the legacy default stream cannot be captured */
+    int32_t reserved;
+} dg_options;
+
+typedef struct {
+    int32_t N, J, K, Np, Nfp;
+    int32_t T;        /* K^tri: boundary triangles */
+    int32_t E;        /* K^lin: boundary lines */
+    int32_t C;        /* K^pnt: corners */
+    int32_t precision;
+    int32_t launches_per_step; /* kernels launched by one time step (5 LSRK stages) */
+    double dt;
+    uint64_t device_bytes;     /* device memory held by the solver */
+} dg_info;
+
+/* Device bytes dg_create needs for this problem (lets the caller allocate the workspace, e.g. with torch). */
+int dg_workspace_bytes(const dg_mesh* mesh, int N, int J, int precision, uint64_t* bytes);
+
+/* Build the solver: mesh hierarchy, reference operators (Warp & Blend nodes, D_r/D_s/D_t, LIFT; PAPER.md:L489,
+ * L529), geometric factors, Padé coefficients c_n (eq (6)), inverse edge / corner matrices (L475), and
+ * upload.  c, rho: [ntets], constant per cell.  opt == NULL: fp64, cfl 1, default stream,
+ * device 0, CUDA graph on.  All fields start at zero. */
+int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* rho, const dg_options* opt,
+              dg_solver** out);
+
+int dg_get_info(const dg_solver* s, dg_info* out);
+
+/* Physical coordinates of the nodes, [K][Np] each. */
+int dg_get_nodes(const dg_solver* s, double* x, double* y, double* z);
+
+/* Set p,u,v,w ([K][Np] each) and zero every auxiliary field (reading R5); the cached
+ * incoming characteristics are initialised by running the closure chain once on the device. */
+int dg_set_initial(dg_solver* s, const double* p, const double* u, const double* v, const double* w);
+
+/* Advance nsteps time steps of 5 LSRK stages each (eq (42)-(43), L531-540; kernel order L627). Asynchronous. */
+int dg_step(dg_solver* s, int nsteps);
+
+/* Read back the volume fields ([K][Np] each; any pointer may be NULL) and, optionally, the PHYSICAL auxiliary
+ * fields:  face_aux [T][J][3][Nfp] = p_i00 (eq (29)) and the two tangential velocities (in-plane Cartesian
+ * axes in increasing order);  edge_aux [E][J*J][2][N+1] = p_ij0 (eq (32)) and the tangential velocity, set
+ * index i*J+j with i <-> the face of lower normal axis.  Synchronises the stream. */
+int dg_get_fields(dg_solver* s, double* p, double* u, double* v, double* w, double* face_aux, double* edge_aux);
+
+/* Where the auxiliary cells are: per triangle (parent tet, local face, normal axis, outward sign), [T] each;
+ * face_xyz [T][Nfp][3] node coordinates.  Any pointer may be NULL. */
+int dg_get_face_map(const dg_solver* s, int32_t* tet, int32_t* face, int32_t* axis, int32_t* sign, double* face_xyz);
+
+/* Per line: tangent axis [E], the two normal axes [E][2] (lower first) with outward signs [E][2];
+ * edge_xyz [E][N+1][3] node coordinates.  Any pointer may be NULL. */
+int dg_get_edge_map(const dg_solver* s, int32_t* axis, int32_t* normal_axes, int32_t* signs, double* edge_xyz);
+
+/* Reference operators as the library computes them (host only, no device needed): rst [Np][dim],
+ * D [dim][Np][Np] row-major, LIFT [Np][Nfaces*Nfp], Fmask [Nfaces][Nfp].  Any pointer may be NULL.
+ * Returns Np through *np_out. */
+int dg_reference_element(int dim, int N, double* rst, double* D, double* LIFT, int32_t* Fmask, int32_t* np_out);
+
+/* Host-side hierarchy sizes without touching the device: counts[0..3] = K, T, E, C. */
+int dg_mesh_counts(const dg_mesh* mesh, int32_t* counts);
+
+/* Seconds of device time spent in each kernel family during the last dg_profile_step call (one time step run
+ * with CUDA events around every launch; for per-kernel reporting, never inside a timed benchmark region).
+ * ms[0..5] = volume+surface+update 3D, 2D update, 1D update, face closure, edge closure, corner closure. */
+int dg_profile_step(dg_solver* s, double* ms);
+
+const char* dg_last_error(void);
+void dg_destroy(dg_solver* s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DG_HABC_H */

@@ -1,0 +1,180 @@
+"""Thin ctypes binding of include/dg_habc.h — argument marshalling only; every step of the path runs in the
+CUDA kernels of libdg_habc.so.  torch is used for the device workspace and the stream (dg_options)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_LIB = None
+
+
+class DgError(RuntimeError):
+    pass
+
+
+class _Mesh(C.Structure):
+    _fields_ = [("nverts", C.c_int32), ("xyz", C.POINTER(C.c_double)), ("ntets", C.c_int32),
+                ("tets", C.POINTER(C.c_int32))]
+
+
+class _Options(C.Structure):
+    _fields_ = [("precision", C.c_int32), ("cfl", C.c_double), ("dt", C.c_double), ("stream", C.c_void_p),
+                ("device", C.c_int32), ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64),
+                ("use_graph", C.c_int32), ("reserved", C.c_int32)]
+
+
+class _Info(C.Structure):
+    _fields_ = [("N", C.c_int32), ("J", C.c_int32), ("K", C.c_int32), ("Np", C.c_int32), ("Nfp", C.c_int32),
+                ("T", C.c_int32), ("E", C.c_int32), ("C", C.c_int32), ("precision", C.c_int32),
+                ("launches_per_step", C.c_int32), ("dt", C.c_double), ("device_bytes", C.c_uint64)]
+
+
+EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_step",
+           "dg_get_fields", "dg_get_face_map", "dg_get_edge_map", "dg_reference_element", "dg_mesh_counts",
+           "dg_profile_step", "dg_last_error", "dg_destroy"]
+
+
+def lib() -> C.CDLL:
+    """Load (building if the sources are newer) the C-ABI library.  Fails loudly if it cannot be had."""
+    global _LIB
+    if _LIB is None:
+        path = _build.LIB
+        if _build.is_stale():
+            path = _build.build()
+        _LIB = C.CDLL(path)
+        _LIB.dg_last_error.restype = C.c_char_p
+        _LIB.dg_destroy.restype = None
+        for name in EXPORTS:
+            getattr(_LIB, name)
+    return _LIB
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise DgError(f"[{rc}] " + lib().dg_last_error().decode())
+
+
+def _dp(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ip(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_int32))
+
+
+def _mesh(verts, tets):
+    verts = np.ascontiguousarray(verts, dtype=np.float64)
+    tets = np.ascontiguousarray(tets, dtype=np.int32)
+    return _Mesh(verts.shape[0], _dp(verts), tets.shape[0], _ip(tets)), (verts, tets)
+
+
+def dg_reference_element(dim: int, N: int):
+    """(rst [Np,dim], D [dim,Np,Np], LIFT [Np,Nfaces*Nfp], Fmask [Nfaces,Nfp]) as the library computes them."""
+    Np = {1: N + 1, 2: (N + 1) * (N + 2) // 2, 3: (N + 1) * (N + 2) * (N + 3) // 6}[dim]
+    Nfp = {1: 1, 2: N + 1, 3: (N + 1) * (N + 2) // 2}[dim]
+    nf = dim + 1
+    rst, D = np.empty((Np, dim)), np.empty((dim, Np, Np))
+    LIFT, Fm = np.empty((Np, nf * Nfp)), np.empty((nf, Nfp), dtype=np.int32)
+    npo = C.c_int32(0)
+    _check(lib().dg_reference_element(dim, N, _dp(rst), _dp(D), _dp(LIFT), _ip(Fm), C.byref(npo)))
+    assert npo.value == Np
+    return rst, D, LIFT, Fm
+
+
+def dg_mesh_counts(verts, tets):
+    m, keep = _mesh(verts, tets)
+    out = np.zeros(4, dtype=np.int32)
+    _check(lib().dg_mesh_counts(C.byref(m), _ip(out)))
+    return tuple(int(x) for x in out)
+
+
+class Solver:
+    """dg_create / dg_set_initial / dg_step / dg_get_fields / dg_destroy of the C ABI."""
+
+    def __init__(self, verts, tets, N: int, J: int, c, rho, precision: int = 64, cfl: float = 1.0,
+                 dt: float = 0.0, device: int = 0, use_graph: bool = True, torch_workspace: bool = True):
+        import torch                                          # device memory + stream only
+        if not torch.cuda.is_available():
+            raise DgError("no CUDA device: the DG+HABC path has no CPU fallback")
+        L = lib()
+        m, self._keep = _mesh(verts, tets)
+        c = np.ascontiguousarray(c, dtype=np.float64)
+        rho = np.ascontiguousarray(rho, dtype=np.float64)
+        opt = _Options()
+        opt.precision, opt.cfl, opt.dt, opt.device, opt.use_graph = precision, cfl, dt, device, int(use_graph)
+        self._torch = torch
+        torch.cuda.set_device(device)
+        # a dedicated (capturable) torch stream: the solver's kernels and CUDA graph run on it
+        self._stream = torch.cuda.Stream(device=device)
+        self.stream = self._stream
+        opt.stream = self._stream.cuda_stream
+        self._ws = None
+        if torch_workspace:
+            nbytes = C.c_uint64(0)
+            _check(L.dg_workspace_bytes(C.byref(m), N, J, precision, C.byref(nbytes)))
+            self._ws = torch.empty(int(nbytes.value), dtype=torch.uint8, device=f"cuda:{device}")
+            opt.workspace_dev, opt.workspace_bytes = self._ws.data_ptr(), nbytes.value
+        self._h = C.c_void_p()
+        _check(L.dg_create(C.byref(m), N, J, _dp(c), _dp(rho), C.byref(opt), C.byref(self._h)))
+        info = _Info()
+        _check(L.dg_get_info(self._h, C.byref(info)))
+        self.info = {k: getattr(info, k) for k, _ in _Info._fields_}
+        for k, v in self.info.items():
+            setattr(self, k, v)
+
+    # ---- boundary calls
+    def get_nodes(self):
+        x = np.empty((3, self.K, self.Np))
+        _check(lib().dg_get_nodes(self._h, _dp(x[0]), _dp(x[1]), _dp(x[2])))
+        return x[0], x[1], x[2]
+
+    def set_initial(self, p, u, v, w):
+        a = [np.ascontiguousarray(f, dtype=np.float64).reshape(self.K, self.Np) for f in (p, u, v, w)]
+        _check(lib().dg_set_initial(self._h, *[_dp(f) for f in a]))
+
+    def step(self, nsteps: int = 1):
+        _check(lib().dg_step(self._h, int(nsteps)))
+
+    def get_fields(self, aux: bool = True):
+        q = np.empty((4, self.K, self.Np))
+        fa = np.zeros((self.T, self.J, 3, self.Nfp)) if aux else None
+        ea = np.zeros((self.E, self.J * self.J, 2, self.N + 1)) if aux else None
+        _check(lib().dg_get_fields(self._h, _dp(q[0]), _dp(q[1]), _dp(q[2]), _dp(q[3]), _dp(fa), _dp(ea)))
+        return q, fa, ea
+
+    def get_face_map(self):
+        tet, face, axis, sign = (np.empty(self.T, dtype=np.int32) for _ in range(4))
+        xyz = np.empty((self.T, self.Nfp, 3))
+        _check(lib().dg_get_face_map(self._h, _ip(tet), _ip(face), _ip(axis), _ip(sign), _dp(xyz)))
+        return tet, face, axis, sign, xyz
+
+    def get_edge_map(self):
+        axis = np.empty(self.E, dtype=np.int32)
+        nax, sg = np.empty((self.E, 2), dtype=np.int32), np.empty((self.E, 2), dtype=np.int32)
+        xyz = np.empty((self.E, self.N + 1, 3))
+        _check(lib().dg_get_edge_map(self._h, _ip(axis), _ip(nax), _ip(sg), _dp(xyz)))
+        return axis, nax, sg, xyz
+
+    def profile_step(self):
+        ms = np.zeros(6)
+        _check(lib().dg_profile_step(self._h, _dp(ms)))
+        return dict(zip(("vol3d", "face2d", "edge1d", "close_face", "close_edge", "close_corner"), ms.tolist()))
+
+    def synchronize(self):
+        self._stream.synchronize()
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().dg_destroy(self._h)
+            self._h = C.c_void_p()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,720 @@
+// C ABI of the DG + HABC time stepper (include/dg_habc.h): host setup, device upload, stage sequencing.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <set>
+#include <stdexcept>
+#include <string>
+#include <vector>
+
+#include "../../include/dg_habc.h"
+#include "habc_coef.hpp"
+#include "kernels.cuh"
+#include "kernels_aux.cuh"
+#include "mesh.hpp"
+
+namespace {
+
+thread_local std::string g_err;
+
+int set_err(int code, const std::string& msg) { g_err = msg; return code; }
+
+int err_from_exception(const std::exception& e) {
+    std::string m = e.what();
+    if (m.rfind("EMESH", 0) == 0) return set_err(DG_EMESH, m);
+    if (m.rfind("ECUDA", 0) == 0) return set_err(DG_ECUDA, m);
+    if (m.rfind("ENOMEM", 0) == 0) return set_err(DG_ENOMEM, m);
+    return set_err(DG_EINVAL, m);
+}
+
+void cu(cudaError_t e, const char* what) {
+    if (e != cudaSuccess) throw std::runtime_error(std::string("ECUDA: ") + what + ": " + cudaGetErrorString(e));
+}
+
+// LSRK4(5) of Carpenter & Kennedy (ref. [10] of the paper; eq (42)-(43))
+const double RKA[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
+                       -3550918686646.0 / 2091501179385.0, -1275806237668.0 / 842570457699.0};
+const double RKB[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 13612068292357.0,
+                       1720146321549.0 / 2090206949498.0, 3134564353537.0 / 4481467310338.0,
+                       2277821191437.0 / 14882151754819.0};
+
+struct Arena {
+    char* base = nullptr;
+    size_t size = 0, used = 0;
+    bool dry = true;
+    void* take(size_t bytes) {
+        size_t o = (used + 255) & ~size_t(255);
+        used = o + bytes;
+        if (dry) return nullptr;
+        if (used > size) throw std::runtime_error("ENOMEM: workspace too small");
+        return base + o;
+    }
+};
+
+}  // namespace
+
+struct dg_solver {
+    dg::HostMesh m;
+    dg::HabcCoef hc;
+    int N = 0, J = 0, precision = 64, device = 0;
+    double dt = 0;
+    cudaStream_t stream = nullptr;
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    bool own_ws = false;
+    dg::Dev<double> d64{};
+    dg::Dev<float> d32{};
+    int cur = 0;
+    int grid3 = 0;
+    size_t smem3 = 0;
+    bool use_graph = true;
+    cudaGraphExec_t graph[2] = {nullptr, nullptr};
+    std::vector<double> rho, c;
+    double* export_buf = nullptr;   // device scratch for dg_get_fields (aux fields, fp64)
+    size_t export_elems = 0;
+};
+
+namespace {
+
+using namespace dg;
+
+// ---------------------------------------------------------------- device image of the problem
+template <typename T>
+struct Uploader {
+    Arena& A;
+    cudaStream_t st;
+    template <typename S>
+    const T* real(const std::vector<S>& h, size_t n) {
+        T* p = (T*)A.take(sizeof(T) * std::max<size_t>(n, 1));
+        if (!A.dry && h.size() != n) throw std::runtime_error("EINVAL: internal size mismatch");
+        if (!A.dry && !h.empty()) {
+            std::vector<T> t(h.begin(), h.end());
+            cu(cudaMemcpy(p, t.data(), sizeof(T) * t.size(), cudaMemcpyHostToDevice), "upload");
+        }
+        return p;
+    }
+    template <typename I, typename S>
+    const I* ints(const std::vector<S>& h, size_t n) {
+        I* p = (I*)A.take(sizeof(I) * std::max<size_t>(n, 1));
+        if (!A.dry && h.size() != n) throw std::runtime_error("EINVAL: internal size mismatch");
+        if (!A.dry && !h.empty()) {
+            std::vector<I> t(h.begin(), h.end());
+            cu(cudaMemcpy(p, t.data(), sizeof(I) * t.size(), cudaMemcpyHostToDevice), "upload");
+        }
+        return p;
+    }
+    T* zeros(size_t n) {
+        T* p = (T*)A.take(sizeof(T) * std::max<size_t>(n, 1));
+        if (!A.dry) cu(cudaMemset(p, 0, sizeof(T) * std::max<size_t>(n, 1)), "memset");
+        return p;
+    }
+};
+
+// Sizes only (dry run) or the real upload.  `s` must hold the host mesh, coefficients, rho, c.
+template <typename T>
+void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
+    const HostMesh& m = s->m;
+    const int K = m.K, Tn = s->J > 0 ? m.T : 0, E = s->J > 0 ? m.E : 0, C = s->J > 0 ? m.C : 0;
+    const int Np = m.Np, Nfp = m.Nfp, N1 = m.N1, J = s->J;
+    Uploader<T> U{A, s->stream};
+    d.N = m.N; d.J = J; d.K = K; d.Tn = Tn; d.E = E; d.C = C; d.Np = Np; d.Nfp = Nfp; d.N1 = N1;
+    d.invM = T(1.0 / (2 * J + 1));
+    // ---- 3D state
+    const size_t n3 = (size_t)K * Np * 4;
+    d.q[0] = U.zeros(n3); d.q[1] = U.zeros(n3); d.res = U.zeros(n3);
+    std::vector<double> geo, dt3, lt3;
+    std::vector<int> fm3;
+    std::vector<uint32_t> finfo;
+    if (!A.dry) {
+        geo.assign((size_t)K * GEO3, 0.0);
+        finfo.assign(K, 0);
+        for (int k = 0; k < K; ++k) {
+            double* g = &geo[(size_t)k * GEO3];
+            for (int q = 0; q < 9; ++q) g[q] = m.G3[(size_t)k * 9 + q];
+            const double Zm = s->rho[k] * s->c[k];
+            for (int f = 0; f < 4; ++f) {
+                const int nb = m.nbr3[(size_t)k * 4 + f];
+                const double Zp = nb >= 0 ? s->rho[nb] * s->c[nb] : Zm;
+                const double Fs = m.Fs3[(size_t)k * 4 + f];
+                g[9 + f] = Zp / ((Zp + Zm) * Fs);
+                g[13 + f] = 1.0 / (Zp + Zm);
+                g[17 + f] = Fs;
+                finfo[k] |= (uint32_t)(m.nbrface3[(size_t)k * 4 + f] | (m.nbrperm3[(size_t)k * 4 + f] << 2)) << (8 * f);
+            }
+            g[21] = s->rho[k] * s->c[k] * s->c[k];
+            g[22] = 1.0 / s->rho[k];
+            g[23] = s->c[k];
+        }
+        dt3.resize((size_t)3 * Np * Np);
+        for (int a = 0; a < 3; ++a)
+            for (int n = 0; n < Np; ++n)
+                for (int q = 0; q < Np; ++q) dt3[((size_t)a * Np + q) * Np + n] = m.r3.D[a][(size_t)n * Np + q];
+        lt3.resize((size_t)4 * Nfp * Np);
+        for (int n = 0; n < Np; ++n)
+            for (int j = 0; j < 4 * Nfp; ++j) lt3[(size_t)j * Np + n] = m.r3.LIFT[(size_t)n * 4 * Nfp + j];
+        fm3.assign(m.r3.Fmask.begin(), m.r3.Fmask.end());
+    }
+    d.geo3 = U.real(geo, (size_t)K * GEO3);
+    d.nbr3 = U.template ints<int>(m.nbr3, (size_t)K * 4);
+    d.finfo3 = U.template ints<uint32_t>(finfo, K);
+    d.Dt3 = U.real(dt3, (size_t)3 * Np * Np); d.Lt3 = U.real(lt3, (size_t)4 * Nfp * Np);
+    d.fmask3 = U.template ints<short>(fm3, 4 * Nfp);
+    d.perm3 = U.template ints<uint8_t>(m.perm3, 6 * Nfp);
+    // ---- 2D
+    const size_t n2 = (size_t)Tn * J * 3 * Nfp;
+    d.fa[0] = U.zeros(n2); d.fa[1] = U.zeros(n2); d.fres = U.zeros(n2);
+    d.S2 = U.zeros((size_t)std::max(m.T, 1) * Nfp);
+    d.qb3 = U.zeros((size_t)std::max(m.T, 1) * Nfp);
+    std::vector<double> geo2, d2, l2;
+    std::vector<int> fm2;
+    if (!A.dry) {
+        geo2.assign((size_t)m.T * GEO2, 0.0); d2.resize((size_t)2 * Nfp * Nfp);
+        for (int t = 0; t < m.T; ++t) {
+            double* g = &geo2[(size_t)t * GEO2];
+            const int k = m.tri_tet[t];
+            const double Zm = s->rho[k] * s->c[k];
+            for (int q = 0; q < 4; ++q) g[q] = m.G2[(size_t)t * 4 + q];
+            for (int q = 0; q < 6; ++q) g[4 + q] = m.n2[(size_t)t * 6 + q];
+            for (int e = 0; e < 3; ++e) {
+                g[10 + e] = m.Fs2[(size_t)t * 3 + e];
+                const int nb = m.nbr2[(size_t)t * 3 + e];
+                double Zp = Zm;
+                if (nb >= 0) { const int kn = m.tri_tet[nb]; Zp = s->rho[kn] * s->c[kn]; }
+                g[13 + e] = Zp / (Zp + Zm);
+                g[16 + e] = 1.0 / (Zp + Zm);
+            }
+            g[19] = s->rho[k] * s->c[k] * s->c[k]; g[20] = 1.0 / s->rho[k]; g[21] = s->c[k]; g[22] = Zm;
+        }
+        for (int a = 0; a < 2; ++a)
+            for (size_t q = 0; q < (size_t)Nfp * Nfp; ++q) d2[(size_t)a * Nfp * Nfp + q] = m.r2.D[a][q];
+        l2 = m.r2.LIFT;
+        fm2.assign(m.r2.Fmask.begin(), m.r2.Fmask.end());
+    }
+    d.geo2 = U.real(geo2, (size_t)m.T * GEO2);
+    d.nbr2 = U.template ints<int>(m.nbr2, (size_t)m.T * 3);
+    d.nbrnode2 = U.template ints<int>(m.nbrnode2, (size_t)m.T * 3 * N1);
+    d.tri_tet = U.template ints<int>(m.tri_tet, m.T);
+    d.tri_face = U.template ints<int>(m.tri_face, m.T);
+    d.tri_axis = U.template ints<int>(m.tri_axis, m.T);
+    d.tri_sign = U.template ints<int>(m.tri_sign, m.T);
+    d.D2 = U.real(d2, (size_t)2 * Nfp * Nfp); d.L2 = U.real(l2, (size_t)Nfp * 3 * N1);
+    d.fmask2 = U.template ints<short>(fm2, 3 * N1);
+    // ---- 1D
+    const size_t n1 = (size_t)E * J * J * 2 * N1;
+    d.ea[0] = U.zeros(n1); d.ea[1] = U.zeros(n1); d.eres = U.zeros(n1);
+    d.S1 = U.zeros((size_t)std::max(m.E, 1) * 2 * std::max(J, 1) * N1);
+    d.qb2 = U.zeros((size_t)std::max(m.E, 1) * 2 * std::max(J, 1) * N1);
+    std::vector<double> geo1;
+    std::vector<int> slot, osign;
+    if (!A.dry) {
+        geo1.assign((size_t)m.E * GEO1, 0.0); slot.resize((size_t)m.E * 2); osign.resize((size_t)m.E * 2);
+        for (int l = 0; l < m.E; ++l) {
+            double* g = &geo1[(size_t)l * GEO1];
+            const int k = m.tri_tet[m.lin_tri[l * 2]];                 // material of the triangle on face A (reading R9)
+            const double Zm = s->rho[k] * s->c[k];
+            g[0] = 1.0 / m.J1[l];
+            for (int e = 0; e < 2; ++e) {
+                const int nb = m.nbr1[l * 2 + e];
+                double Zp = Zm;
+                if (nb >= 0) { const int kn = m.tri_tet[m.lin_tri[nb * 2]]; Zp = s->rho[kn] * s->c[kn]; }
+                g[1 + e] = Zp / (Zp + Zm);
+                g[3 + e] = 1.0 / (Zp + Zm);
+            }
+            g[5] = s->rho[k] * s->c[k] * s->c[k]; g[6] = 1.0 / s->rho[k]; g[7] = s->c[k];
+            for (int side = 0; side < 2; ++side) {
+                const int t = m.lin_tri[l * 2 + side], oth = m.lin_ab[l * 2 + 1 - side];
+                slot[l * 2 + side] = (m.tri_ax[t * 2] == oth) ? 0 : 1;
+                osign[l * 2 + side] = m.lin_sign[l * 2 + 1 - side];
+            }
+        }
+    }
+    d.geo1 = U.real(geo1, (size_t)m.E * GEO1);
+    d.nbr1 = U.template ints<int>(m.nbr1, (size_t)m.E * 2);
+    d.lin_tri = U.template ints<int>(m.lin_tri, (size_t)m.E * 2);
+    d.lin_trinode = U.template ints<int>(m.lin_trinode, (size_t)m.E * 2 * N1);
+    d.lin_slot = U.template ints<int>(slot, (size_t)m.E * 2);
+    d.lin_osign = U.template ints<int>(osign, (size_t)m.E * 2);
+    d.D1 = U.real(m.r1.D[0], (size_t)N1 * N1); d.L1 = U.real(m.r1.LIFT, (size_t)N1 * 2);
+    // ---- 0D + algebra
+    d.qb1 = U.zeros((size_t)std::max(m.C, 1) * 3 * std::max(J * J, 1));
+    d.cor_line = U.template ints<int>(m.cor_line, (size_t)m.C * 3);
+    d.cor_end = U.template ints<int>(m.cor_end, (size_t)m.C * 3);
+    d.cor_sign = U.template ints<int>(m.cor_sign, (size_t)m.C * 3);
+    const HabcCoef& h = s->hc;
+    const size_t e2 = (size_t)4 * J * J, c2 = (size_t)9 * J * J * J * J;
+    d.cn = U.real(h.cn, J);
+    d.Cij = U.real(h.Cij, (size_t)J * J);
+    d.Pe = U.real(h.Pe, e2);
+    d.Qe = U.real(h.Qe, e2);
+    d.Gc = U.real(h.Gc, c2);
+    // fp64 scratch for exporting the physical auxiliary fields
+    s->export_elems = n2 + n1;
+    s->export_buf = (double*)A.take(sizeof(double) * std::max<size_t>(s->export_elems, 1));
+}
+
+// ---------------------------------------------------------------- kernel dispatch
+template <typename T, int N, int G, int ET, bool SM>
+void launch_vol3d_cfg(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
+    using Cfg = Vol3dCfg<T, N, G, ET, SM>;
+    auto kern = k_vol3d<T, N, G, ET, SM>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int per_sm = 0, sms = 0;
+        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: volume kernel does not fit on an SM");
+        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
+        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
+}
+
+template <typename T> struct OpsFit;
+template <> struct OpsFit<double> { static constexpr int maxN = 5; };
+template <> struct OpsFit<float> { static constexpr int maxN = 6; };
+
+template <typename T>
+void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
+    constexpr int mx = OpsFit<T>::maxN;
+    switch (s->N) {
+        case 1: launch_vol3d_cfg<T, 1, 32, 4, true>(s, d, src, a, b, configure); break;
+        case 2: launch_vol3d_cfg<T, 2, 16, 4, true>(s, d, src, a, b, configure); break;
+        case 3: launch_vol3d_cfg<T, 3, 8, 4, true>(s, d, src, a, b, configure); break;
+        case 4: launch_vol3d_cfg<T, 4, 8, 4, true>(s, d, src, a, b, configure); break;
+        case 5: launch_vol3d_cfg<T, 5, 4, 4, true>(s, d, src, a, b, configure); break;
+        case 6: launch_vol3d_cfg<T, 6, 4, 2, (6 <= mx)>(s, d, src, a, b, configure); break;
+        case 7: launch_vol3d_cfg<T, 7, 2, 4, false>(s, d, src, a, b, configure); break;
+        case 8: launch_vol3d_cfg<T, 8, 2, 2, false>(s, d, src, a, b, configure); break;
+        default: throw std::runtime_error("EINVAL: N must be in 1..8");
+    }
+}
+
+// one LSRK stage: 3D, 2D, 1D solvers (independent), then the closure chain 2D -> 1D -> 0D
+template <typename T>
+void launch_closures(dg_solver* s, Dev<T>& d, int cur) {
+    if (d.J == 0 || d.Tn == 0) return;
+    const int nf = d.Tn * d.Nfp;
+    k_close_face<T><<<(nf + 255) / 256, 256, 0, s->stream>>>(d, cur);
+    if (d.E > 0) {
+        const int ne = d.E * d.N1;
+        k_close_edge<T><<<(ne + 63) / 64, 64, 0, s->stream>>>(d, cur);
+    }
+    if (d.C > 0) {
+        const int JJ3 = 3 * d.J * d.J;
+        k_close_corner<T><<<d.C, std::min(1024, ((JJ3 + 31) / 32) * 32), sizeof(T) * JJ3, s->stream>>>(d, cur);
+    }
+}
+
+template <typename T>
+void launch_stage(dg_solver* s, Dev<T>& d, int src, int stage) {
+    const double a = RKA[stage], b = RKB[stage];
+    launch_vol3d<T>(s, d, src, a, b, false);
+    if (d.J > 0 && d.Tn > 0) {
+        const int nt = ((std::max(d.Nfp, 3 * d.N1) + 31) / 32) * 32;
+        k_face2d<T><<<d.Tn, nt, sizeof(T) * (3 * d.Nfp + 3 * d.N1), s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
+        if (d.E > 0) {
+            const int work = d.J * d.J * d.N1;
+            k_edge1d<T><<<d.E, std::min(512, ((work + 31) / 32) * 32), sizeof(T) * 2 * work, s->stream>>>(
+                d, src, (T)a, (T)b, (T)s->dt);
+        }
+    }
+    launch_closures<T>(s, d, src ^ 1);
+}
+
+int launches_per_stage(const dg_solver* s) {
+    int n = 1;
+    if (s->J > 0 && s->m.T > 0) {
+        n += 2;                       // 2D solver + face closure
+        if (s->m.E > 0) n += 2;       // 1D solver + edge closure
+        if (s->m.C > 0) n += 1;       // corner closure
+    }
+    return n;
+}
+
+template <typename T>
+void run_step_plain(dg_solver* s, Dev<T>& d) {
+    for (int st = 0; st < 5; ++st) {
+        launch_stage<T>(s, d, s->cur, st);
+        s->cur ^= 1;
+    }
+}
+
+template <typename T>
+void run_steps(dg_solver* s, Dev<T>& d, int nsteps) {
+    if (!s->use_graph) {
+        for (int i = 0; i < nsteps; ++i) run_step_plain<T>(s, d);
+        cu(cudaGetLastError(), "kernel launch");
+        return;
+    }
+    for (int i = 0; i < nsteps; ++i) {
+        const int par = s->cur;
+        if (!s->graph[par]) {
+            cudaGraph_t g;
+            cu(cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal), "begin capture");
+            run_step_plain<T>(s, d);
+            cu(cudaStreamEndCapture(s->stream, &g), "end capture");
+            cu(cudaGraphInstantiate(&s->graph[par], g, 0), "graph instantiate");
+            cudaGraphDestroy(g);
+            s->cur = par;              // capture did not execute anything
+        }
+        cu(cudaGraphLaunch(s->graph[par], s->stream), "graph launch");
+        s->cur = par ^ 1;              // five stages flip the parity once
+    }
+}
+
+size_t dry_bytes(dg_solver* s) {
+    Arena A;
+    A.dry = true;
+    if (s->precision == 64) { Dev<double> d{}; build_device<double>(s, A, d); }
+    else { Dev<float> d{}; build_device<float>(s, A, d); }
+    return A.used + 256;
+}
+
+void check_args(const dg_mesh* mesh, int N, int J, int precision) {
+    if (!mesh || !mesh->xyz || !mesh->tets) throw std::runtime_error("EINVAL: NULL mesh");
+    if (N < 1 || N > 8) throw std::runtime_error("EINVAL: N must be in 1..8");
+    if (J < 0 || J > JMAX) throw std::runtime_error("EINVAL: J must be in 0..12");
+    if (precision != 64 && precision != 32) throw std::runtime_error("EINVAL: precision must be 64 or 32");
+}
+
+template <typename T>
+void upload_initial(dg_solver* s, Dev<T>& d, const double* p, const double* u, const double* v, const double* w) {
+    const size_t n = (size_t)d.K * d.Np;
+    std::vector<T> h(n * 4);
+    for (size_t i = 0; i < n; ++i) {
+        h[i * 4] = (T)p[i]; h[i * 4 + 1] = (T)u[i]; h[i * 4 + 2] = (T)v[i]; h[i * 4 + 3] = (T)w[i];
+    }
+    cu(cudaMemcpyAsync(d.q[0], h.data(), sizeof(T) * h.size(), cudaMemcpyHostToDevice, s->stream), "upload q");
+    cu(cudaMemsetAsync(d.q[1], 0, sizeof(T) * n * 4, s->stream), "memset");
+    cu(cudaMemsetAsync(d.res, 0, sizeof(T) * n * 4, s->stream), "memset");
+    const size_t n2 = (size_t)d.Tn * d.J * 3 * d.Nfp, n1 = (size_t)d.E * d.J * d.J * 2 * d.N1;
+    for (int b = 0; b < 2; ++b) {
+        if (n2) cu(cudaMemsetAsync(d.fa[b], 0, sizeof(T) * n2, s->stream), "memset");
+        if (n1) cu(cudaMemsetAsync(d.ea[b], 0, sizeof(T) * n1, s->stream), "memset");
+    }
+    if (n2) cu(cudaMemsetAsync(d.fres, 0, sizeof(T) * n2, s->stream), "memset");
+    if (n1) cu(cudaMemsetAsync(d.eres, 0, sizeof(T) * n1, s->stream), "memset");
+    s->cur = 0;
+    launch_closures<T>(s, d, 0);        // reading R5: cached r^-, S consistent with the initial state
+    cu(cudaStreamSynchronize(s->stream), "set_initial");
+}
+
+template <typename T>
+void download_fields(dg_solver* s, Dev<T>& d, double* p, double* u, double* v, double* w, double* fa, double* ea) {
+    const size_t n = (size_t)d.K * d.Np;
+    if (p || u || v || w) {
+        std::vector<T> h(n * 4);
+        cu(cudaMemcpyAsync(h.data(), d.q[s->cur], sizeof(T) * h.size(), cudaMemcpyDeviceToHost, s->stream), "download q");
+        cu(cudaStreamSynchronize(s->stream), "sync");
+        for (size_t i = 0; i < n; ++i) {
+            if (p) p[i] = (double)h[i * 4];
+            if (u) u[i] = (double)h[i * 4 + 1];
+            if (v) v[i] = (double)h[i * 4 + 2];
+            if (w) w[i] = (double)h[i * 4 + 3];
+        }
+    }
+    const size_t n2 = (size_t)d.Tn * d.J * 3 * d.Nfp, n1 = (size_t)d.E * d.J * d.J * 2 * d.N1;
+    if ((fa || ea) && n2 + n1 > 0) {
+        const size_t tot = n2 + n1;
+        k_export_aux<T><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(d, s->cur, s->export_buf, s->export_buf + n2);
+        cu(cudaGetLastError(), "export launch");
+        if (fa && n2) cu(cudaMemcpyAsync(fa, s->export_buf, sizeof(double) * n2, cudaMemcpyDeviceToHost, s->stream), "download");
+        if (ea && n1) cu(cudaMemcpyAsync(ea, s->export_buf + n2, sizeof(double) * n1, cudaMemcpyDeviceToHost, s->stream), "download");
+    }
+    cu(cudaStreamSynchronize(s->stream), "sync");
+}
+
+template <typename T>
+void profile_step(dg_solver* s, Dev<T>& d, double* ms) {
+    for (int i = 0; i < 6; ++i) ms[i] = 0;
+    cudaEvent_t ev[2];
+    cu(cudaEventCreate(&ev[0]), "event"); cu(cudaEventCreate(&ev[1]), "event");
+    auto timed = [&](int slot, auto&& fn) {
+        cu(cudaEventRecord(ev[0], s->stream), "record");
+        fn();
+        cu(cudaEventRecord(ev[1], s->stream), "record");
+        cu(cudaEventSynchronize(ev[1]), "sync");
+        float t = 0;
+        cu(cudaEventElapsedTime(&t, ev[0], ev[1]), "elapsed");
+        ms[slot] += t;
+    };
+    for (int st = 0; st < 5; ++st) {
+        const int src = s->cur;
+        const double a = RKA[st], b = RKB[st];
+        timed(0, [&] { launch_vol3d<T>(s, d, src, a, b, false); });
+        if (d.J > 0 && d.Tn > 0) {
+            const int nt = ((std::max(d.Nfp, 3 * d.N1) + 31) / 32) * 32;
+            timed(1, [&] {
+                k_face2d<T><<<d.Tn, nt, sizeof(T) * (3 * d.Nfp + 3 * d.N1), s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
+            });
+            if (d.E > 0) {
+                const int work = d.J * d.J * d.N1;
+                timed(2, [&] {
+                    k_edge1d<T><<<d.E, std::min(512, ((work + 31) / 32) * 32), sizeof(T) * 2 * work, s->stream>>>(
+                        d, src, (T)a, (T)b, (T)s->dt);
+                });
+            }
+            const int cur = src ^ 1;
+            timed(3, [&] { k_close_face<T><<<(d.Tn * d.Nfp + 255) / 256, 256, 0, s->stream>>>(d, cur); });
+            if (d.E > 0) timed(4, [&] { k_close_edge<T><<<(d.E * d.N1 + 63) / 64, 64, 0, s->stream>>>(d, cur); });
+            if (d.C > 0) {
+                const int JJ3 = 3 * d.J * d.J;
+                timed(5, [&] {
+                    k_close_corner<T><<<d.C, std::min(1024, ((JJ3 + 31) / 32) * 32), sizeof(T) * JJ3, s->stream>>>(d, cur);
+                });
+            }
+        }
+        s->cur ^= 1;
+    }
+    cudaEventDestroy(ev[0]); cudaEventDestroy(ev[1]);
+    cu(cudaGetLastError(), "profile step");
+}
+
+}  // namespace
+
+// ======================================================================================= C ABI
+extern "C" {
+
+const char* dg_last_error(void) { return g_err.c_str(); }
+
+int dg_mesh_counts(const dg_mesh* mesh, int32_t* counts) {
+    try {
+        if (!mesh || !counts) throw std::runtime_error("EINVAL: NULL argument");
+        dg::HostMesh m;
+        dg::build_mesh(m, 1, mesh->nverts, mesh->xyz, mesh->ntets, mesh->tets);
+        counts[0] = m.K; counts[1] = m.T; counts[2] = m.E; counts[3] = m.C;
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+int dg_reference_element(int dim, int N, double* rst, double* D, double* LIFT, int32_t* Fmask, int32_t* np_out) {
+    try {
+        dg::RefElem e = dg::make_refelem(dim, N);
+        if (np_out) *np_out = e.Np;
+        if (rst) for (size_t i = 0; i < e.rst.size(); ++i) rst[i] = (double)e.rst[i];
+        if (D) for (int a = 0; a < dim; ++a) std::copy(e.D[a].begin(), e.D[a].end(), D + (size_t)a * e.Np * e.Np);
+        if (LIFT) std::copy(e.LIFT.begin(), e.LIFT.end(), LIFT);
+        if (Fmask) std::copy(e.Fmask.begin(), e.Fmask.end(), Fmask);
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+// Exact hierarchy sizes of a cuboid mesh without building connectivity: boundary cell faces are the faces whose
+// three vertices share a bounding plane; boundary lines are the distinct cell edges lying on two bounding planes.
+static void quick_counts(const dg_mesh* mesh, int& T, int& E) {
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int v = 0; v < mesh->nverts; ++v)
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = std::min(lo[d], mesh->xyz[v * 3 + d]);
+            hi[d] = std::max(hi[d], mesh->xyz[v * 3 + d]);
+        }
+    const double tol = 1e-9 * std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]});
+    std::vector<uint8_t> code(mesh->nverts, 0);
+    for (int v = 0; v < mesh->nverts; ++v)
+        for (int d = 0; d < 3; ++d) {
+            if (std::fabs(mesh->xyz[v * 3 + d] - lo[d]) < tol) code[v] |= 1 << (2 * d);
+            if (std::fabs(mesh->xyz[v * 3 + d] - hi[d]) < tol) code[v] |= 2 << (2 * d);
+        }
+    T = 0;
+    std::set<std::pair<int, int>> lines;
+    for (int k = 0; k < mesh->ntets; ++k) {
+        const int32_t* t = mesh->tets + (size_t)k * 4;
+        for (int f = 0; f < 4; ++f) {
+            int a = t[dg::TET_FACE_VERTS[f][0]], b = t[dg::TET_FACE_VERTS[f][1]], c = t[dg::TET_FACE_VERTS[f][2]];
+            if (code[a] & code[b] & code[c]) ++T;
+        }
+        for (int i = 0; i < 4; ++i)
+            for (int j = i + 1; j < 4; ++j)
+                if (__builtin_popcount(code[t[i]] & code[t[j]]) >= 2)
+                    lines.insert({std::min(t[i], t[j]), std::max(t[i], t[j])});
+    }
+    E = (int)lines.size();
+}
+
+int dg_workspace_bytes(const dg_mesh* mesh, int N, int J, int precision, uint64_t* bytes) {
+    try {
+        check_args(mesh, N, J, precision);
+        if (!bytes) throw std::runtime_error("EINVAL: NULL argument");
+        dg_solver s;
+        s.N = N; s.J = J; s.precision = precision;
+        s.m.N = N; s.m.K = mesh->ntets; s.m.C = 8;
+        quick_counts(mesh, s.m.T, s.m.E);
+        s.m.Np = (N + 1) * (N + 2) * (N + 3) / 6; s.m.Nfp = (N + 1) * (N + 2) / 2; s.m.N1 = N + 1;
+        *bytes = dry_bytes(&s) + 4096;
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* rho, const dg_options* opt,
+              dg_solver** out) {
+    dg_solver* s = nullptr;
+    try {
+        const int precision = opt ? opt->precision : 64;
+        check_args(mesh, N, J, precision);
+        if (!c || !rho || !out) throw std::runtime_error("EINVAL: NULL argument");
+        for (int k = 0; k < mesh->ntets; ++k)
+            if (!(c[k] > 0) || !(rho[k] > 0)) throw std::runtime_error("EINVAL: c and rho must be positive");
+        s = new dg_solver();
+        s->N = N; s->J = J; s->precision = precision;
+        s->device = opt ? opt->device : 0;
+        s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
+        s->use_graph = opt ? opt->use_graph != 0 : true;
+        if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured
+        s->rho.assign(rho, rho + mesh->ntets);
+        s->c.assign(c, c + mesh->ntets);
+        dg::build_mesh(s->m, N, mesh->nverts, mesh->xyz, mesh->ntets, mesh->tets);
+        s->hc = dg::make_habc(J);
+        // eq (46), PAPER.md:L796 (reading R7): dt = cfl * min_k 1 / (c_k (N+1)^2 max_f Fscale_kf)
+        double dtmin = 1e300;
+        for (int k = 0; k < s->m.K; ++k) {
+            double fs = 0;
+            for (int f = 0; f < 4; ++f) fs = std::max(fs, s->m.Fs3[(size_t)k * 4 + f]);
+            dtmin = std::min(dtmin, 1.0 / (c[k] * (N + 1) * (N + 1) * fs));
+        }
+        const double cfl = (opt && opt->cfl > 0) ? opt->cfl : 1.0;
+        s->dt = (opt && opt->dt > 0) ? opt->dt : cfl * dtmin;
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        const size_t need = dry_bytes(s);
+        if (opt && opt->workspace_dev) {
+            if (opt->workspace_bytes < need) throw std::runtime_error("ENOMEM: workspace_bytes is smaller than dg_workspace_bytes");
+            s->ws = opt->workspace_dev; s->ws_bytes = opt->workspace_bytes; s->own_ws = false;
+        } else {
+            if (cudaMalloc(&s->ws, need) != cudaSuccess) { cudaGetLastError(); throw std::runtime_error("ENOMEM: cudaMalloc failed"); }
+            s->ws_bytes = need; s->own_ws = true;
+        }
+        Arena A;
+        A.base = (char*)s->ws; A.size = s->ws_bytes; A.dry = false;
+        // align the arena base to 256 B
+        size_t mis = (size_t)(uintptr_t)A.base & 255;
+        if (mis) { A.base += 256 - mis; A.size -= 256 - mis; }
+        if (precision == 64) { build_device<double>(s, A, s->d64); launch_vol3d<double>(s, s->d64, 0, 0, 0, true); }
+        else { build_device<float>(s, A, s->d32); launch_vol3d<float>(s, s->d32, 0, 0, 0, true); }
+        cu(cudaDeviceSynchronize(), "setup");
+        *out = s;
+        return DG_OK;
+    } catch (const std::exception& e) {
+        if (s) dg_destroy(s);
+        return err_from_exception(e);
+    }
+}
+
+void dg_destroy(dg_solver* s) {
+    if (!s) return;
+    for (int i = 0; i < 2; ++i) if (s->graph[i]) cudaGraphExecDestroy(s->graph[i]);
+    if (s->own_ws && s->ws) cudaFree(s->ws);
+    delete s;
+}
+
+int dg_get_info(const dg_solver* s, dg_info* o) {
+    if (!s || !o) return set_err(DG_EINVAL, "EINVAL: NULL argument");
+    o->N = s->N; o->J = s->J; o->K = s->m.K; o->Np = s->m.Np; o->Nfp = s->m.Nfp;
+    o->T = s->m.T; o->E = s->m.E; o->C = s->m.C; o->precision = s->precision;
+    o->launches_per_step = 5 * launches_per_stage(s);
+    o->dt = s->dt; o->device_bytes = s->ws_bytes;
+    return DG_OK;
+}
+
+int dg_get_nodes(const dg_solver* s, double* x, double* y, double* z) {
+    if (!s) return set_err(DG_EINVAL, "EINVAL: NULL argument");
+    const dg::HostMesh& m = s->m;
+    double* out[3] = {x, y, z};
+    for (int k = 0; k < m.K; ++k)
+        for (int n = 0; n < m.Np; ++n)
+            for (int d = 0; d < 3; ++d) {
+                if (!out[d]) continue;
+                long double acc = 0;
+                for (int v = 0; v < 4; ++v) acc += m.r3.bary[(size_t)n * 4 + v] * m.verts[(size_t)m.tets[(size_t)k * 4 + v] * 3 + d];
+                out[d][(size_t)k * m.Np + n] = (double)acc;
+            }
+    return DG_OK;
+}
+
+int dg_set_initial(dg_solver* s, const double* p, const double* u, const double* v, const double* w) {
+    try {
+        if (!s || !p || !u || !v || !w) throw std::runtime_error("EINVAL: NULL argument");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        if (s->precision == 64) upload_initial<double>(s, s->d64, p, u, v, w);
+        else upload_initial<float>(s, s->d32, p, u, v, w);
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+int dg_step(dg_solver* s, int nsteps) {
+    try {
+        if (!s || nsteps < 0) throw std::runtime_error("EINVAL: bad argument");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        if (s->precision == 64) run_steps<double>(s, s->d64, nsteps);
+        else run_steps<float>(s, s->d32, nsteps);
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+int dg_get_fields(dg_solver* s, double* p, double* u, double* v, double* w, double* face_aux, double* edge_aux) {
+    try {
+        if (!s) throw std::runtime_error("EINVAL: NULL argument");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        if (s->precision == 64) download_fields<double>(s, s->d64, p, u, v, w, face_aux, edge_aux);
+        else download_fields<float>(s, s->d32, p, u, v, w, face_aux, edge_aux);
+        cu(cudaGetLastError(), "device work");
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+int dg_get_face_map(const dg_solver* s, int32_t* tet, int32_t* face, int32_t* axis, int32_t* sign, double* xyz) {
+    if (!s) return set_err(DG_EINVAL, "EINVAL: NULL argument");
+    const dg::HostMesh& m = s->m;
+    for (int t = 0; t < m.T; ++t) {
+        if (tet) tet[t] = m.tri_tet[t];
+        if (face) face[t] = m.tri_face[t];
+        if (axis) axis[t] = m.tri_axis[t];
+        if (sign) sign[t] = m.tri_sign[t];
+        if (xyz)
+            for (int j = 0; j < m.Nfp; ++j) {
+                const int n = m.r3.Fmask[m.tri_face[t] * m.Nfp + j];
+                for (int d = 0; d < 3; ++d) {
+                    long double acc = 0;
+                    for (int v = 0; v < 4; ++v)
+                        acc += m.r3.bary[(size_t)n * 4 + v] * m.verts[(size_t)m.tets[(size_t)m.tri_tet[t] * 4 + v] * 3 + d];
+                    xyz[((size_t)t * m.Nfp + j) * 3 + d] = (double)acc;
+                }
+            }
+    }
+    return DG_OK;
+}
+
+int dg_get_edge_map(const dg_solver* s, int32_t* axis, int32_t* normal_axes, int32_t* signs, double* xyz) {
+    if (!s) return set_err(DG_EINVAL, "EINVAL: NULL argument");
+    const dg::HostMesh& m = s->m;
+    for (int l = 0; l < m.E; ++l) {
+        if (axis) axis[l] = m.lin_axis[l];
+        for (int q = 0; q < 2; ++q) {
+            if (normal_axes) normal_axes[l * 2 + q] = m.lin_ab[l * 2 + q];
+            if (signs) signs[l * 2 + q] = m.lin_sign[l * 2 + q];
+        }
+        if (xyz)
+            for (int n = 0; n < m.N1; ++n)
+                for (int d = 0; d < 3; ++d) {
+                    long double acc = 0;
+                    for (int v = 0; v < 2; ++v) acc += m.r1.bary[(size_t)n * 2 + v] * m.verts[(size_t)m.lin_v[l * 2 + v] * 3 + d];
+                    xyz[((size_t)l * m.N1 + n) * 3 + d] = (double)acc;
+                }
+    }
+    return DG_OK;
+}
+
+int dg_profile_step(dg_solver* s, double* ms) {
+    try {
+        if (!s || !ms) throw std::runtime_error("EINVAL: NULL argument");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        if (s->precision == 64) profile_step<double>(s, s->d64, ms);
+        else profile_step<float>(s, s->d32, ms);
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+}  // extern "C"

@@ -1,0 +1,83 @@
+"""Shared harness of the parity tests: run the oracle and the CUDA library on the same seeded workload and
+compare element by element (cells matched by centroid, nodes by coordinates).  Imports both sides; neither
+side imports the other."""
+from __future__ import annotations
+
+import numpy as np
+
+
+def _cell_order(x):
+    c = np.round(x.mean(axis=1) * 1e7).astype(np.int64)
+    return np.lexsort(c.T)
+
+
+def match_cells(xa, xb, tol=1e-9):
+    """xa, xb [n, nodes, 3] the same cells in different cell / node orders.  Returns (ia, ib, perm) such that
+    xa[ia][:, k] == xb[ib][np.arange(n)[:,None], perm][:, k]."""
+    ia, ib = _cell_order(xa), _cell_order(xb)
+    A, B = xa[ia], xb[ib]
+    d = np.abs(A[:, :, None, :] - B[:, None, :, :]).max(axis=3)
+    perm = np.argmin(d, axis=2)
+    assert np.take_along_axis(d, perm[:, :, None], axis=2).max() < tol, "cells do not match"
+    return ia, ib, perm
+
+
+def rel_l2(a, b):
+    nb = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / nb) if nb > 0 else float(np.linalg.norm(a))
+
+
+def initial_on(w, x, y, z, c_elem, rho_elem):
+    cn = np.repeat(np.asarray(c_elem)[:, None], x.shape[1], axis=1)
+    rn = np.repeat(np.asarray(rho_elem)[:, None], x.shape[1], axis=1)
+    return w.fields(x, y, z, cn, rn)
+
+
+def run_oracle(w, nsteps=None, dt=None):
+    from oracle.solver import OracleSolver
+    o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho, dt=dt)
+    x = o.nodes()
+    o.set_initial(np.stack(initial_on(w, x[..., 0], x[..., 1], x[..., 2], w.c, w.rho)))
+    o.step(w.nsteps if nsteps is None else nsteps)
+    q, fa, ea = o.get_fields()
+    return dict(dt=o.dt, x=x, q=q, fa=fa, ea=ea, xf=o.H.tri.x if o.T else np.zeros((0, 1, 3)),
+                xe=o.H.lin.x if o.E else np.zeros((0, 1, 3)), T=o.T, E=o.E, C=o.C)
+
+
+def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True):
+    from paper_1610_05023_b200 import Solver
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=precision, dt=dt, use_graph=use_graph)
+    x, y, z = s.get_nodes()
+    s.set_initial(*initial_on(w, x, y, z, w.c, w.rho))
+    s.step(w.nsteps if nsteps is None else nsteps)
+    q, fa, ea = s.get_fields()
+    _, _, _, _, xf = s.get_face_map()
+    _, _, _, xe = s.get_edge_map()
+    out = dict(dt=s.dt, x=np.stack([x, y, z], axis=-1), q=q, fa=fa, ea=ea, xf=xf, xe=xe, T=s.T, E=s.E, C=s.C,
+               info=s.info)
+    s.close()
+    return out
+
+
+def compare(lib, ora):
+    """Relative L2 error per field group (BASELINE north_star: p, u and all auxiliary fields)."""
+    ia, ib, perm = match_cells(lib["x"], ora["x"])
+    rows = np.arange(len(ia))[:, None]
+    ql = lib["q"][:, ia]
+    qo = ora["q"][:, ib][:, rows, perm]
+    out = {"p": rel_l2(ql[0], qo[0]), "u": rel_l2(ql[1:], qo[1:]),
+           "norm_p": float(np.linalg.norm(qo[0])), "norm_u": float(np.linalg.norm(qo[1:]))}
+    if ora["T"] and ora["fa"].size:
+        ia, ib, perm = match_cells(lib["xf"], ora["xf"])
+        rows = np.arange(len(ia))[:, None]
+        fl = lib["fa"][ia]                                            # [T,J,3,Nfp]
+        fo = np.take_along_axis(ora["fa"][ib], perm[:, None, None, :], axis=3)
+        out["face"] = rel_l2(fl, fo)
+        out["norm_face"] = float(np.linalg.norm(fo))
+    if ora["E"] and ora["ea"].size:
+        ia, ib, perm = match_cells(lib["xe"], ora["xe"])
+        el = lib["ea"][ia]
+        eo = np.take_along_axis(ora["ea"][ib], perm[:, None, None, :], axis=3)
+        out["edge"] = rel_l2(el, eo)
+        out["norm_edge"] = float(np.linalg.norm(eo))
+    return out
