@@ -1,0 +1,274 @@
+#!/usr/bin/env python
+"""bench.py — DG+HABC node-updates/s on B200 (BASELINE.json metric), with roofline and CPU-oracle baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--precision 64|32] [--impl reference]
+
+One "step" = one full time step (5 LSRK stages, every kernel of SURVEY §8(a)) over the whole synthetic mesh.
+N>1 (torchrun): independent replicas, one per GPU ("replicas only") — weak scaling, no collective
+on the data path.  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from workloads import CONFIGS, make_workload  # noqa: E402
+
+METRIC = "DG+HABC node-updates/sec"
+UNIT = "node-updates/s"
+# measured on this pool's B200 with paper_1610_05023_b200/csrc/ubench/peaks.cu (profiles/r01_peaks.md)
+FP64_TFLOPS_MEASURED = 34.0
+FP32_TFLOPS_MEASURED = 72.0
+HBM_FALLBACK_GBS = 6650.0
+
+
+def algorithmic_bytes_per_element(N: int, precision: int) -> float:
+    """per element and LSRK stage the 3D kernel must move q,res in and out (16 Np values), the
+    neighbours' face traces (4 fields x 4 Nfp values), 24 geometric/material values, and 20 B of connectivity."""
+    Np, Nfp = (N + 1) * (N + 2) * (N + 3) // 6, (N + 1) * (N + 2) // 2
+    return (precision // 8) * (16 * Np + 16 * Nfp + 24) + 20
+
+
+def algorithmic_flops_per_element(N: int) -> float:
+    """DESIGN.md §7 (minimal operation count): 6 matvec rows per node (12 Np flop), 24 flop to form the
+    contravariant velocity and combine the gradient, LIFT on one flux scalar per face node (8 Nfp per node),
+    ~14 flop per face node for the flux, 40 per node for the face combination + update."""
+    Np, Nfp = (N + 1) * (N + 2) * (N + 3) // 6, (N + 1) * (N + 2) // 2
+    return Np * (12 * Np + 24 + 8 * Nfp + 40) + 4 * Nfp * 14
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.max = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max,
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+def oracle_sample(workload: str, precision: int, budget_s: float = 20.0):
+    """Time the oracle (as it stands) on a bounded sample of the workload: same N, J, materials rule, pulse, on a
+    coarser hex grid (n=8), for as many steps as fit the budget.  Returns (node-updates/s, description, cores)."""
+    from oracle.solver import OracleSolver
+    d = CONFIGS[workload]
+    n = min(d["n"], 8)
+    w = make_workload(workload, n=n)
+    o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho)
+    x = o.nodes()
+    cn = np.repeat(w.c[:, None], x.shape[1], axis=1)
+    o.set_initial(np.stack(w.fields(x[..., 0], x[..., 1], x[..., 2], cn, 1.0)))
+    o.step(1)
+    steps, t0 = 0, time.perf_counter()
+    while True:
+        o.step(1)
+        steps += 1
+        el = time.perf_counter() - t0
+        if el > budget_s or steps >= 50:
+            break
+    nodes = o.H.tet.K * o.H.tet.ref.Np
+    cores = len(os.sched_getaffinity(0))
+    desc = f"{workload} rule on a {n}^3 hex grid ({o.H.tet.K} tets, N={w.N}, J={w.J}), {steps} steps, fp64 numpy"
+    return nodes * steps / el, desc, cores, el / steps
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    per_step_budget = 6.0
+    vals = []
+    for _ in range(args.warmup + args.steps):
+        v, desc, cores, step_s = oracle_sample(args.workload, 64, budget_s=per_step_budget)
+        vals.append((v, step_s))
+    vals = vals[args.warmup:]
+    value = float(np.mean([v for v, _ in vals]))
+    d = CONFIGS[args.workload]
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([s for _, s in vals])),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "n_hex": d["n"], "N": d["N"], "J": d["J"]},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--precision", type=int, default=64)
+    ap.add_argument("--n", type=int, default=None, help="override hexes per side (debug only; invalidates the metric)")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1610_05023_b200 import Solver
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = make_workload(args.workload, n=args.n)
+    prec = args.precision
+    t_setup = time.perf_counter()
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local)
+    x, y, z = s.get_nodes()
+    cn = np.repeat(w.c[:, None], s.Np, axis=1)
+    fields = [np.ascontiguousarray(f) for f in w.fields(x, y, z, cn, 1.0)]
+    del x, y, z
+    s.set_initial(*fields)
+    t_setup = time.perf_counter() - t_setup
+    nodes = s.K * s.Np
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput
+    s.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(s.stream):
+        ev0.record(s.stream)
+        s.step(args.steps)
+        ev1.record(s.stream)
+    barrier()
+    sampler.stop_flag = True
+    ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * nodes * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel device time (outside the timed region): the dominant kernel's roofline
+    prof = {k: 0.0 for k in ("vol3d", "face2d", "edge1d", "close_face", "close_edge", "close_corner")}
+    nprof = 3
+    for _ in range(nprof):
+        for k, v in s.profile_step().items():
+            prof[k] += v / nprof
+    vol_ms = prof["vol3d"] / 5.0                                  # per launch
+    bytes_launch = algorithmic_bytes_per_element(w.N, prec) * s.K
+    flops_launch = algorithmic_flops_per_element(w.N) * s.K
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
+    alu_peak = FP64_TFLOPS_MEASURED if prec == 64 else FP32_TFLOPS_MEASURED
+    hbm = {"bound": "hbm", "achieved": bytes_launch / (vol_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+           "peak_source": "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback"}
+    hbm["frac"] = hbm["achieved"] / hbm["peak"]
+    alu = {"bound": "alu", "achieved": flops_launch / (vol_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+           "peak_source": "profiles/r01_peaks.md (DFMA/FFMA microbenchmark on this pool)"}
+    alu["frac"] = alu["achieved"] / alu["peak"]
+    t_mem, t_alu = bytes_launch / (hbm_peak * 1e9), flops_launch / (alu_peak * 1e12)
+    roof = dict(hbm if t_mem >= t_alu else alu)
+    roof.update({"kernel": "k_vol3d", "ms_per_launch": vol_ms, "traffic": None,
+                 "roof_ms": 1e3 * max(t_mem, t_alu), "frac_of_slower_roof": max(t_mem, t_alu) / (vol_ms * 1e-3),
+                 "hbm": hbm, "alu": alu, "kernel_share_of_step": prof["vol3d"] / max(sum(prof.values()), 1e-12),
+                 "per_kernel_ms_per_step": prof})
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        try:
+            roof["traffic"] = json.load(open(traffic_file)).get(f"{args.workload}_f{prec}")
+        except Exception:
+            pass
+
+    # ---- end to end through the C ABI with host buffers: H2D of the fields, the steps, D2H of the fields
+    barrier()
+    t0 = time.perf_counter()
+    s.set_initial(*fields)
+    s.step(args.steps)
+    q, _, _ = s.get_fields(aux=False)
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = 4 * nodes * (prec // 8)
+    e2e = {"value": world * nodes * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d / args.steps,
+           "d2h_bytes_per_step": h2d / args.steps, "seconds": e2e_s,
+           "what": "dg_set_initial(host) + dg_step(steps) + dg_get_fields(host), wall clock"}
+    finite = bool(np.isfinite(q).all())
+    launches = s.launches_per_step * args.steps
+    info = dict(s.info)
+    s.close()
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": f"f{prec}", "data": "synthetic",
+            "config": {"workload": args.workload, "n_hex": w.n, "N": w.N, "J": w.J, "K": info["K"], "T": info["T"],
+                       "E": info["E"], "corners": info["C"], "nodes": nodes, "dt": info["dt"],
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "state (q,res) exceeds L2 many times over; no flush needed",
+                       "setup_s": t_setup, "finite": finite},
+            "node_stages_per_s": 5 * value, "roofline": roof, "e2e": e2e, "gpu_launches": launches,
+            "clocks": sampler.summary()}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, desc, cores, _ = oracle_sample(args.workload, prec)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,106 @@
+"""Parity tests proper (-m gpu): the CUDA path through the C ABI against the oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json north_star's: relative L2 <= 1e-11 (fp64), <= 1e-4 (fp32) on
+p, u and every auxiliary field."""
+import numpy as np
+import pytest
+
+import parity
+from workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+TOL = {64: 1e-11, 32: 1e-4}
+
+
+def _check(err, prec, aux=True):
+    groups = ["p", "u"] + (["face", "edge"] if aux else [])
+    for k in groups:
+        assert err[k] <= TOL[prec], (k, err)
+    if aux:      # pin P16: the auxiliary levels really carry data (non-vacuous parity)
+        assert err["norm_face"] > 1e-3 * err["norm_p"] and err["norm_edge"] > 1e-4 * err["norm_p"], err
+
+
+def test_cfg1_full_fp64():
+    """BASELINE configs[0]: 48 tets, N=3, J=2, 100 steps."""
+    w = make_workload("cfg1")
+    lib, ora = parity.run_library(w), parity.run_oracle(w)
+    assert lib["dt"] == pytest.approx(ora["dt"], rel=1e-14)
+    assert (lib["T"], lib["E"], lib["C"]) == (48, 24, 8)
+    _check(parity.compare(lib, ora), 64)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_cfg2_reduced_steps(prec):
+    """BASELINE configs[1] (3,072 tets, N=4, J=4, Gaussian + plane wave) for 60 of its 500 steps (the full count
+    is run by tests/test_gpu_full_configs.py)."""
+    w = make_workload("cfg2")
+    lib, ora = parity.run_library(w, precision=prec, nsteps=60), parity.run_oracle(w, nsteps=60)
+    _check(parity.compare(lib, ora), prec)
+
+
+def test_cfg3_shape_perturbed_layered():
+    """configs[2] recipe (perturbed interior vertices, 4 layers of c in U[1,3], N=4, J=6) on a 6^3 hex grid:
+    several batches of the persistent kernel plus a ragged tail (1296 tets = 40 batches of 32 + 16)."""
+    w = make_workload("cfg3", n=6, nsteps=40)
+    assert np.unique(w.c).size == 4
+    lib, ora = parity.run_library(w), parity.run_oracle(w)
+    _check(parity.compare(lib, ora), 64)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_cfg5_shape(prec):
+    """configs[4] recipe (N=5, J=8, layered c in U[1.5,4.5]) on a 5^3 hex grid (750 tets: ragged tail of 14)."""
+    w = make_workload("cfg5", n=5, nsteps=30)
+    lib, ora = parity.run_library(w, precision=prec), parity.run_oracle(w)
+    _check(parity.compare(lib, ora), prec)
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("J", [0, 4])
+def test_cfg4_degree_sweep(N, J):
+    """configs[3]: every degree N=1..8 with J in {0,4} (J=8 in test_J8_degree below) on a 3^3 hex grid."""
+    w = make_workload("cfg4", n=3, N=N, J=J, nsteps=10)
+    lib, ora = parity.run_library(w), parity.run_oracle(w)
+    _check(parity.compare(lib, ora), 64, aux=J > 0)
+
+
+@pytest.mark.parametrize("N", [2, 6])
+def test_J8_degree(N):
+    w = make_workload("cfg4", n=2, N=N, J=8, nsteps=10)
+    for prec in (64, 32):
+        lib, ora = parity.run_library(w, precision=prec), parity.run_oracle(w)
+        _check(parity.compare(lib, ora), prec)
+
+
+def test_edge_cases():
+    """Smallest mesh (one hex, 6 tets: every tet touches the boundary), J=1, J=12 (maximum), graph off,
+    negatively oriented input cells, zero initial data, nsteps=0."""
+    w = make_workload("cfg1", n=1, N=2, J=1, nsteps=15)
+    _check(parity.compare(parity.run_library(w), parity.run_oracle(w)), 64)
+    w = make_workload("cfg1", n=1, N=1, J=12, nsteps=15)
+    _check(parity.compare(parity.run_library(w, use_graph=False), parity.run_oracle(w)), 64)
+    # flipped vertex order in half the cells: same solution
+    w = make_workload("cfg1", nsteps=10)
+    ora = parity.run_oracle(w)
+    w.tets = w.tets.copy()
+    w.tets[::2] = w.tets[::2][:, [0, 1, 3, 2]]
+    _check(parity.compare(parity.run_library(w), ora), 64)
+    # nsteps = 0 returns the initial data; zero data stays zero
+    lib = parity.run_library(w, nsteps=0)
+    x = lib["x"]
+    p0 = w.fields(x[..., 0], x[..., 1], x[..., 2], 1.0, 1.0)[0]
+    assert np.abs(lib["q"][0] - p0).max() == 0.0
+    from paper_1610_05023_b200 import Solver
+    s = Solver(w.verts, w.tets, 3, 2, w.c, w.rho)
+    s.step(3)
+    q, fa, ea = s.get_fields()
+    assert not q.any() and not fa.any() and not ea.any()
+    s.close()
+
+
+def test_missing_device_is_loud(monkeypatch):
+    import torch
+    from paper_1610_05023_b200 import DgError, Solver
+    monkeypatch.setattr(torch.cuda, "is_available", lambda: False)
+    w = make_workload("cfg1")
+    with pytest.raises(DgError):
+        Solver(w.verts, w.tets, 3, 2, w.c, w.rho)
