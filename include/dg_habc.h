@@ -56,7 +56,8 @@ typedef struct {
     uint64_t workspace_bytes; /* size of workspace_dev; see dg_workspace_bytes */
     int32_t use_graph;        /* 1: replay the 5-stage step as a CUDA graph; ignored (plain launches) when stream is NULL,
                                  because the legacy default stream cannot be captured */
-    int32_t reserved;
+    int32_t kernel;           /* 3D kernel: 0 = the library's choice; 1 = scalar-FMA kernel (any N, fp64/fp32);
+                                 2 = fp64 tensor-pipe (DMMA) kernel, N <= 5 only (DG_EINVAL otherwise) */
 } dg_options;
 
 typedef struct {

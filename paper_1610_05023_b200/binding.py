@@ -24,7 +24,7 @@ class _Mesh(C.Structure):
 class _Options(C.Structure):
     _fields_ = [("precision", C.c_int32), ("cfl", C.c_double), ("dt", C.c_double), ("stream", C.c_void_p),
                 ("device", C.c_int32), ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64),
-                ("use_graph", C.c_int32), ("reserved", C.c_int32)]
+                ("use_graph", C.c_int32), ("kernel", C.c_int32)]
 
 
 class _Info(C.Structure):
@@ -96,7 +96,8 @@ class Solver:
     """dg_create / dg_set_initial / dg_step / dg_get_fields / dg_destroy of the C ABI."""
 
     def __init__(self, verts, tets, N: int, J: int, c, rho, precision: int = 64, cfl: float = 1.0,
-                 dt: float = 0.0, device: int = 0, use_graph: bool = True, torch_workspace: bool = True):
+                 dt: float = 0.0, device: int = 0, use_graph: bool = True, torch_workspace: bool = True,
+                 kernel: int = 0):
         import torch                                          # device memory + stream only
         if not torch.cuda.is_available():
             raise DgError("no CUDA device: the DG+HABC path has no CPU fallback")
@@ -106,6 +107,7 @@ class Solver:
         rho = np.ascontiguousarray(rho, dtype=np.float64)
         opt = _Options()
         opt.precision, opt.cfl, opt.dt, opt.device, opt.use_graph = precision, cfl, dt, device, int(use_graph)
+        opt.kernel = int(kernel)
         self._torch = torch
         torch.cuda.set_device(device)
         # a dedicated (capturable) torch stream: the solver's kernels and CUDA graph run on it

@@ -7,6 +7,7 @@
 #include <map>
 #include <set>
 #include <stdexcept>
+#include <type_traits>
 #include <string>
 #include <vector>
 
@@ -14,6 +15,7 @@
 #include "habc_coef.hpp"
 #include "kernels.cuh"
 #include "kernels_aux.cuh"
+#include "kernel_vol3d_mma.cuh"
 #include "mesh.hpp"
 
 namespace {
@@ -70,6 +72,8 @@ struct dg_solver {
     int cur = 0;
     int grid3 = 0;
     size_t smem3 = 0;
+    int kernel = 0;                 // dg_options.kernel as requested
+    bool mma3 = false;              // the tensor-pipe 3D kernel is in use
     bool use_graph = true;
     cudaGraphExec_t graph[2] = {nullptr, nullptr};
     std::vector<double> rho, c;
@@ -127,10 +131,11 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.q[0] = U.zeros(n3); d.q[1] = U.zeros(n3); d.res = U.zeros(n3);
     std::vector<double> geo, dt3, lt3;
     std::vector<int> fm3;
-    std::vector<uint32_t> finfo;
+    std::vector<uint32_t> finfo, conn;
     if (!A.dry) {
         geo.assign((size_t)K * GEO3, 0.0);
         finfo.assign(K, 0);
+        conn.assign((size_t)K * 4, 0);
         for (int k = 0; k < K; ++k) {
             double* g = &geo[(size_t)k * GEO3];
             for (int q = 0; q < 9; ++q) g[q] = m.G3[(size_t)k * 9 + q];
@@ -142,7 +147,9 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
                 g[9 + f] = Zp / ((Zp + Zm) * Fs);
                 g[13 + f] = 1.0 / (Zp + Zm);
                 g[17 + f] = Fs;
-                finfo[k] |= (uint32_t)(m.nbrface3[(size_t)k * 4 + f] | (m.nbrperm3[(size_t)k * 4 + f] << 2)) << (8 * f);
+                const uint32_t fp = (uint32_t)(m.nbrface3[(size_t)k * 4 + f] | (m.nbrperm3[(size_t)k * 4 + f] << 2));
+                finfo[k] |= fp << (8 * f);
+                conn[(size_t)k * 4 + f] = nb >= 0 ? ((uint32_t)nb << 5) | fp : CONN_BND | ((uint32_t)(-1 - nb) << 5);
             }
             g[21] = s->rho[k] * s->c[k] * s->c[k];
             g[22] = 1.0 / s->rho[k];
@@ -160,6 +167,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.geo3 = U.real(geo, (size_t)K * GEO3);
     d.nbr3 = U.template ints<int>(m.nbr3, (size_t)K * 4);
     d.finfo3 = U.template ints<uint32_t>(finfo, K);
+    d.conn3 = U.template ints<uint32_t>(conn, (size_t)K * 4);
     d.Dt3 = U.real(dt3, (size_t)3 * Np * Np); d.Lt3 = U.real(lt3, (size_t)4 * Nfp * Np);
     d.fmask3 = U.template ints<short>(fm3, 4 * Nfp);
     d.perm3 = U.template ints<uint8_t>(m.perm3, 6 * Nfp);
@@ -278,9 +286,44 @@ template <typename T> struct OpsFit;
 template <> struct OpsFit<double> { static constexpr int maxN = 5; };
 template <> struct OpsFit<float> { static constexpr int maxN = 6; };
 
+// fp64 tensor-pipe kernel (kernel_vol3d_mma.cuh): degrees whose A fragments fit the register file
+constexpr int MMA_MAX_N = 5;
+
+template <int N>
+void launch_vol3d_mma_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    using Cfg = MmaCfg<N>;
+    auto kern = k_vol3d_mma<N>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int per_sm = 0, sms = 0;
+        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: tensor-pipe volume kernel does not fit on an SM");
+        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
+        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, a, b, s->dt);
+}
+
+void launch_vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    switch (s->N) {
+        case 1: launch_vol3d_mma_cfg<1>(s, d, src, a, b, configure); break;
+        case 2: launch_vol3d_mma_cfg<2>(s, d, src, a, b, configure); break;
+        case 3: launch_vol3d_mma_cfg<3>(s, d, src, a, b, configure); break;
+        case 4: launch_vol3d_mma_cfg<4>(s, d, src, a, b, configure); break;
+        case 5: launch_vol3d_mma_cfg<5>(s, d, src, a, b, configure); break;
+        default: throw std::runtime_error("EINVAL: the tensor-pipe kernel covers N = 1..5");
+    }
+}
+
 template <typename T>
 void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
     constexpr int mx = OpsFit<T>::maxN;
+    if constexpr (std::is_same<T, double>::value) {
+        if (s->mma3) return launch_vol3d_mma(s, d, src, a, b, configure);
+    }
     switch (s->N) {
         case 1: launch_vol3d_cfg<T, 1, 32, 4, true>(s, d, src, a, b, configure); break;
         case 2: launch_vol3d_cfg<T, 2, 16, 4, true>(s, d, src, a, b, configure); break;
@@ -564,6 +607,12 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->device = opt ? opt->device : 0;
         s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
         s->use_graph = opt ? opt->use_graph != 0 : true;
+        s->kernel = opt ? opt->kernel : 0;
+        if (s->kernel < 0 || s->kernel > 2) throw std::runtime_error("EINVAL: dg_options.kernel must be 0, 1 or 2");
+        if (s->kernel == 2 && (precision != 64 || N > MMA_MAX_N))
+            throw std::runtime_error("EINVAL: the tensor-pipe kernel (kernel = 2) covers fp64, N = 1..5");
+        if (mesh->ntets > CONN_MAX_ID) throw std::runtime_error("EINVAL: more than 2^26 - 1 tetrahedra");
+        s->mma3 = precision == 64 && N <= MMA_MAX_N && s->kernel != 1;
         if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured
         s->rho.assign(rho, rho + mesh->ntets);
         s->c.assign(c, c + mesh->ntets);

@@ -29,6 +29,7 @@ struct Dev {
     const T* geo3;                   // [K][GEO3]
     const int* nbr3;                 // [K][4]  neighbour tet or -1-triangle
     const uint32_t* finfo3;          // [K]     byte f: neighbour face | perm << 2
+    const uint32_t* conn3;           // [K][4]  packed (kernel_vol3d_mma.cuh): boundary flag | id << 5 | perm << 2 | face
     const T* Dt3;                    // [3][Np][Np]  Dt3[a][m][n] = D_a[n][m]
     const T* Lt3;                    // [4 Nfp][Np]  Lt3[j][n]   = LIFT[n][j]
     const short* fmask3;             // [4][Nfp]
