@@ -127,15 +127,16 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.N = m.N; d.J = J; d.K = K; d.Tn = Tn; d.E = E; d.C = C; d.Np = Np; d.Nfp = Nfp; d.N1 = N1;
     d.invM = T(1.0 / (2 * J + 1));
     // ---- 3D state
-    const size_t n3 = (size_t)K * Np * 4;
+    const size_t Kp = ((size_t)K + 7) / 8 * 8;     // the tensor-pipe kernel reads whole batches of 8 elements
+    const size_t n3 = Kp * Np * 4;
     d.q[0] = U.zeros(n3); d.q[1] = U.zeros(n3); d.res = U.zeros(n3);
     std::vector<double> geo, dt3, lt3;
     std::vector<int> fm3;
     std::vector<uint32_t> finfo, conn;
     if (!A.dry) {
-        geo.assign((size_t)K * GEO3, 0.0);
+        geo.assign(Kp * GEO3, 0.0);
         finfo.assign(K, 0);
-        conn.assign((size_t)K * 4, 0);
+        conn.assign(Kp * 4, 0);
         for (int k = 0; k < K; ++k) {
             double* g = &geo[(size_t)k * GEO3];
             for (int q = 0; q < 9; ++q) g[q] = m.G3[(size_t)k * 9 + q];
@@ -164,10 +165,10 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
             for (int j = 0; j < 4 * Nfp; ++j) lt3[(size_t)j * Np + n] = m.r3.LIFT[(size_t)n * 4 * Nfp + j];
         fm3.assign(m.r3.Fmask.begin(), m.r3.Fmask.end());
     }
-    d.geo3 = U.real(geo, (size_t)K * GEO3);
+    d.geo3 = U.real(geo, Kp * GEO3);
     d.nbr3 = U.template ints<int>(m.nbr3, (size_t)K * 4);
     d.finfo3 = U.template ints<uint32_t>(finfo, K);
-    d.conn3 = U.template ints<uint32_t>(conn, (size_t)K * 4);
+    d.conn3 = U.template ints<uint32_t>(conn, Kp * 4);
     d.Dt3 = U.real(dt3, (size_t)3 * Np * Np); d.Lt3 = U.real(lt3, (size_t)4 * Nfp * Np);
     d.fmask3 = U.template ints<short>(fm3, 4 * Nfp);
     d.perm3 = U.template ints<uint8_t>(m.perm3, 6 * Nfp);
@@ -176,6 +177,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.fa[0] = U.zeros(n2); d.fa[1] = U.zeros(n2); d.fres = U.zeros(n2);
     d.S2 = U.zeros((size_t)std::max(m.T, 1) * Nfp);
     d.qb3 = U.zeros((size_t)std::max(m.T, 1) * Nfp);
+    d.ghost3 = U.zeros((size_t)std::max(m.T, 1) * Nfp * 4);
     std::vector<double> geo2, d2, l2;
     std::vector<int> fm2;
     if (!A.dry) {

@@ -38,6 +38,7 @@ struct Dev {
     T* fa[2]; T* fres;               // [T][J][3][Nfp]   p*_i, U_xi, U_eta
     T* S2;                           // [T][Nfp]   r^- + r^+ of the 3D field (q0^tet of the paper)
     T* qb3;                          // [T][Nfp]   r^- for the 3D solver     (qb^tet)
+    T* ghost3;                       // [T][Nfp][4] ghost state (2 r^-, 0, 0, 0) behind an HABC face (tensor-pipe kernel)
     const T* geo2;                   // [T][GEO2]
     const int* nbr2;                 // [T][3]
     const int* nbrnode2;             // [T][3][N1]

@@ -178,6 +178,7 @@ __global__ void k_close_face(Dev<T> d, int cur) {
     for (int i = 0; i < d.J; ++i) rm += d.cn[i] * f[(size_t)i * 3 * d.Nfp];
     rm *= d.invM;
     d.qb3[idx] = rm;
+    d.ghost3[(size_t)idx * 4] = T(2) * rm;
     d.S2[idx] = rp + rm;
 }
 
