@@ -16,6 +16,7 @@
 #include "kernels.cuh"
 #include "kernels_aux.cuh"
 #include "kernel_vol3d_mma.cuh"
+#include "kernel_vol3d_ws.cuh"
 #include "mesh.hpp"
 
 namespace {
@@ -74,6 +75,8 @@ struct dg_solver {
     size_t smem3 = 0;
     int kernel = 0;                 // dg_options.kernel as requested
     bool mma3 = false;              // the tensor-pipe 3D kernel is in use
+    bool ws3 = false;               // ... in its warp-specialised form (kernel_vol3d_ws.cuh)
+    const double* geox3 = nullptr;  // [Kp][GX3] per-tet record of the warp-specialised kernel (dt folded in)
     bool use_graph = true;
     cudaGraphExec_t graph[2] = {nullptr, nullptr};
     std::vector<double> rho, c;
@@ -166,6 +169,27 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
         fm3.assign(m.r3.Fmask.begin(), m.r3.Fmask.end());
     }
     d.geo3 = U.real(geo, Kp * GEO3);
+    if (s->ws3) {
+        // record of kernel_vol3d_ws.cuh: G | dt rho c^2, dt/rho, dt c | (Fs n, A)_f | B_f | Fs_f
+        std::vector<double> gx;
+        if (!A.dry) {
+            gx.assign(Kp * GX3, 0.0);
+            static const double NH[4][3] = {{0, 0, -1}, {0, -1, 0}, {1, 1, 1}, {-1, 0, 0}};   // outward, in (r,s,t)
+            for (int k = 0; k < K; ++k) {
+                const double* g = &geo[(size_t)k * GEO3];
+                double* x = &gx[(size_t)k * GX3];
+                for (int q = 0; q < 9; ++q) x[q] = g[q];
+                x[9] = s->dt * g[21]; x[10] = s->dt * g[22]; x[11] = s->dt * g[23];
+                for (int f = 0; f < 4; ++f) {
+                    for (int c = 0; c < 3; ++c) x[12 + 4 * f + c] = NH[f][0] * g[c] + NH[f][1] * g[3 + c] + NH[f][2] * g[6 + c];
+                    x[12 + 4 * f + 3] = g[9 + f];
+                    x[28 + f] = g[13 + f];
+                    x[32 + f] = g[17 + f];
+                }
+            }
+        }
+        s->geox3 = (const double*)U.real(gx, Kp * GX3);
+    }
     d.nbr3 = U.template ints<int>(m.nbr3, (size_t)K * 4);
     d.finfo3 = U.template ints<uint32_t>(finfo, K);
     d.conn3 = U.template ints<uint32_t>(conn, Kp * 4);
@@ -309,7 +333,30 @@ void launch_vol3d_mma_cfg(dg_solver* s, Dev<double>& d, int src, double a, doubl
     kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, a, b, s->dt);
 }
 
+template <int N>
+void launch_vol3d_ws_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    using Cfg = WsCfg<N>;
+    auto kern = k_vol3d_ws<N>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int sms = 0;
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
+        s->grid3 = std::max(1, std::min(nbatch, sms));       // one persistent CTA per SM (it owns the register file)
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, s->geox3, src, a, b);
+}
+
 void launch_vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    if (s->ws3) {
+        switch (s->N) {
+            case 4: return launch_vol3d_ws_cfg<4>(s, d, src, a, b, configure);
+            case 5: return launch_vol3d_ws_cfg<5>(s, d, src, a, b, configure);
+            default: throw std::runtime_error("EINVAL: the warp-specialised kernel covers N = 4, 5");
+        }
+    }
     switch (s->N) {
         case 1: launch_vol3d_mma_cfg<1>(s, d, src, a, b, configure); break;
         case 2: launch_vol3d_mma_cfg<2>(s, d, src, a, b, configure); break;
@@ -587,6 +634,7 @@ int dg_workspace_bytes(const dg_mesh* mesh, int N, int J, int precision, uint64_
         if (!bytes) throw std::runtime_error("EINVAL: NULL argument");
         dg_solver s;
         s.N = N; s.J = J; s.precision = precision;
+        s.ws3 = precision == 64 && N >= 4 && N <= 5;           // upper bound: covers every dg_options.kernel choice
         s.m.N = N; s.m.K = mesh->ntets; s.m.C = 8;
         quick_counts(mesh, s.m.T, s.m.E);
         s.m.Np = (N + 1) * (N + 2) * (N + 3) / 6; s.m.Nfp = (N + 1) * (N + 2) / 2; s.m.N1 = N + 1;
@@ -610,11 +658,14 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
         s->use_graph = opt ? opt->use_graph != 0 : true;
         s->kernel = opt ? opt->kernel : 0;
-        if (s->kernel < 0 || s->kernel > 2) throw std::runtime_error("EINVAL: dg_options.kernel must be 0, 1 or 2");
+        if (s->kernel < 0 || s->kernel > 3) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..3");
+        if (s->kernel == 3 && (precision != 64 || N < 4 || N > 5))
+            throw std::runtime_error("EINVAL: the warp-specialised kernel (kernel = 3) covers fp64, N = 4, 5");
         if (s->kernel == 2 && (precision != 64 || N > MMA_MAX_N))
             throw std::runtime_error("EINVAL: the tensor-pipe kernel (kernel = 2) covers fp64, N = 1..5");
         if (mesh->ntets > CONN_MAX_ID) throw std::runtime_error("EINVAL: more than 2^26 - 1 tetrahedra");
         s->mma3 = precision == 64 && N <= MMA_MAX_N && s->kernel != 1;
+        s->ws3 = s->mma3 && (s->kernel == 3 || (s->kernel == 0 && N == 5));
         if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured
         s->rho.assign(rho, rho + mesh->ntets);
         s->c.assign(c, c + mesh->ntets);

@@ -44,9 +44,9 @@ def run_oracle(w, nsteps=None, dt=None):
                 xe=o.H.lin.x if o.E else np.zeros((0, 1, 3)), T=o.T, E=o.E, C=o.C)
 
 
-def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True):
+def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True, kernel=0):
     from paper_1610_05023_b200 import Solver
-    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=precision, dt=dt, use_graph=use_graph)
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=precision, dt=dt, use_graph=use_graph, kernel=kernel)
     x, y, z = s.get_nodes()
     s.set_initial(*initial_on(w, x, y, z, w.c, w.rho))
     s.step(w.nsteps if nsteps is None else nsteps)
