@@ -66,6 +66,11 @@ __device__ __forceinline__ double2 ldg_nc2(const double* p) {
 template <int R> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(R)); }
 template <int R> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R)); }
 
+// volatile: keeps the written issue order (independent accumulators interleaved) and pins the hand-over point
+__device__ __forceinline__ void dmma884v(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
 __device__ __forceinline__ void bar_sync64(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 __device__ __forceinline__ void bar_arrive64(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
 
@@ -202,8 +207,11 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
                 const bool bnd = (c & CONN_BND) != 0;
                 const double* base = (bnd ? d.ghost3 + id * (Nfp * 4) : qold + id * (Np * 4)) + 2 * h;
                 const int* tab = sNode + (bnd ? 32 : (int)(c & 31)) * Nfp;     // row 32 is the identity
+                int off[Nfp];                                // all table reads first: cp.async is a compiler barrier
 #pragma unroll
-                for (int j = 0; j < Nfp; ++j) cp_async16(dn + (fl * Nfp + j) * 32, base + tab[j]);
+                for (int j = 0; j < Nfp; ++j) off[j] = tab[j];
+#pragma unroll
+                for (int j = 0; j < Nfp; ++j) cp_async16(dn + (fl * Nfp + j) * 32, base + off[j]);
             }
             cp_async_arrive_noinc(&full[s]);
         }
@@ -259,20 +267,22 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
 #pragma unroll
             for (int s_ = 0; s_ < KD; ++s_) {
                 const double b0 = bp[(0 * KPD + 4 * s_) * EB];
-                dmma884(cpr, Ar[s_], b0);
-                dmma884(cps, As[s_], b0);
-                dmma884(cpt, At[s_], b0);
-                dmma884(cvr, Ar[s_], bp[(1 * KPD + 4 * s_) * EB]);
-                dmma884(cvs, As[s_], bp[(2 * KPD + 4 * s_) * EB]);
-                dmma884(cvt, At[s_], bp[(3 * KPD + 4 * s_) * EB]);
+                dmma884v(cpr, Ar[s_], b0);
+                dmma884v(cps, As[s_], b0);
+                dmma884v(cpt, At[s_], b0);
+                dmma884v(cvr, Ar[s_], bp[(1 * KPD + 4 * s_) * EB]);
+                dmma884v(cvs, As[s_], bp[(2 * KPD + 4 * s_) * EB]);
+                dmma884v(cvt, At[s_], bp[(3 * KPD + 4 * s_) * EB]);
+                // half-way: let the partner start, so that the two DMMA streams overlap by about half (one warp
+                // alone can issue a DMMA every ~24 cycles, the unit takes one every 16)
+                if (s_ == KD / 2 && paired && !(w >= 4 && b + (int)gridDim.x >= nbatch)) bar_arrive64(partner_turn);
             }
             const double* gp = sG + t * EB + (g ^ swz(t));
 #pragma unroll
             for (int s_ = 0; s_ < KL; ++s_)
 #pragma unroll
-                for (int f = 0; f < 4; ++f) dmma884(cl[f], AL[f][s_], gp[f * LPAD + 4 * s_ * EB]);
+                for (int f = 0; f < 4; ++f) dmma884v(cl[f], AL[f][s_], gp[f * LPAD + 4 * s_ * EB]);
         }
-        if (paired && !(w >= 4 && b + (int)gridDim.x >= nbatch)) bar_arrive64(partner_turn);
         __syncwarp();
         if (lane == 0) mbar_arrive(&opfree[o]);
         // ---- right-hand side and LSRK update (eq (41)-(43)) of node n, elements 2t, 2t+1 (dt folded into the record)
