@@ -72,6 +72,7 @@ struct dg_solver {
     dg::Dev<float> d32{};
     int cur = 0;
     int grid3 = 0;
+    int face_grid = 148 * 8;        // persistent CTAs of the 2D solver kernel (set from the SM count in dg_create)
     size_t smem3 = 0;
     int kernel = 0;                 // dg_options.kernel as requested
     bool mma3 = false;              // the tensor-pipe 3D kernel is in use
@@ -386,6 +387,15 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool con
     }
 }
 
+template <typename T>
+void launch_face2d(dg_solver* s, Dev<T>& d, int src, double a, double b) {
+    const int Nf = 3 * d.N1, PB = std::max(1, FACE2D_NT / std::max(d.Nfp, Nf));
+    const size_t smem = sizeof(T) * (2 * d.Nfp * d.Nfp + Nf * d.Nfp + PB * (3 * d.Nfp + Nf));
+    const int nchunk = (d.Tn * d.J + PB - 1) / PB;
+    const int grid = std::max(1, std::min(nchunk, s->face_grid));
+    k_face2d<T><<<grid, FACE2D_NT, smem, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
+}
+
 // one LSRK stage: 3D, 2D, 1D solvers (independent), then the closure chain 2D -> 1D -> 0D
 template <typename T>
 void launch_closures(dg_solver* s, Dev<T>& d, int cur) {
@@ -407,8 +417,7 @@ void launch_stage(dg_solver* s, Dev<T>& d, int src, int stage) {
     const double a = RKA[stage], b = RKB[stage];
     launch_vol3d<T>(s, d, src, a, b, false);
     if (d.J > 0 && d.Tn > 0) {
-        const int nt = ((std::max(d.Nfp, 3 * d.N1) + 31) / 32) * 32;
-        k_face2d<T><<<d.Tn, nt, sizeof(T) * (3 * d.Nfp + 3 * d.N1), s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
+        launch_face2d<T>(s, d, src, a, b);
         if (d.E > 0) {
             const int work = d.J * d.J * d.N1;
             k_edge1d<T><<<d.E, std::min(512, ((work + 31) / 32) * 32), sizeof(T) * 2 * work, s->stream>>>(
@@ -540,10 +549,7 @@ void profile_step(dg_solver* s, Dev<T>& d, double* ms) {
         const double a = RKA[st], b = RKB[st];
         timed(0, [&] { launch_vol3d<T>(s, d, src, a, b, false); });
         if (d.J > 0 && d.Tn > 0) {
-            const int nt = ((std::max(d.Nfp, 3 * d.N1) + 31) / 32) * 32;
-            timed(1, [&] {
-                k_face2d<T><<<d.Tn, nt, sizeof(T) * (3 * d.Nfp + 3 * d.N1), s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
-            });
+            timed(1, [&] { launch_face2d<T>(s, d, src, a, b); });
             if (d.E > 0) {
                 const int work = d.J * d.J * d.N1;
                 timed(2, [&] {
@@ -681,6 +687,11 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         const double cfl = (opt && opt->cfl > 0) ? opt->cfl : 1.0;
         s->dt = (opt && opt->dt > 0) ? opt->dt : cfl * dtmin;
         cu(cudaSetDevice(s->device), "cudaSetDevice");
+        {
+            int sms = 0;
+            cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+            s->face_grid = sms * 8;
+        }
         const size_t need = dry_bytes(s);
         if (opt && opt->workspace_dev) {
             if (opt->workspace_bytes < need) throw std::runtime_error("ENOMEM: workspace_bytes is smaller than dg_workspace_bytes");

@@ -7,75 +7,92 @@
 namespace dg {
 
 // ---------------------------------------------------------------------------------------------------
-// 2D: one CTA per boundary triangle, thread <-> node, loop over the J sets (operators reused, L631).
+// 2D: the J face solvers (operators reused across sets, L631).
 // eq (31a-c): (1+c_i) dt p*_i + rho c^2 div_par U_i = 0 ; rho dt U_i + grad_par p_i = 0, p_i = p*_i + S.
 // ---------------------------------------------------------------------------------------------------
+// Threads <-> (pair, node), pair = (triangle t, set i): FACE2D_NT / max(Nfp, 3 N1) pairs per pass of a persistent CTA, the
+// operators D_r, D_s, LIFT2D staged once per CTA in shared memory (transposed: lanes <-> consecutive nodes).
+constexpr int FACE2D_NT = 128;
+
 template <typename T>
-__global__ void k_face2d(Dev<T> d, int src, T rka, T rkb, T dt) {
+__global__ void __launch_bounds__(FACE2D_NT) k_face2d(Dev<T> d, int src, T rka, T rkb, T dt) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* sp = reinterpret_cast<T*>(smem_raw);       // [Nfp]
-    const int Nfp = d.Nfp, N1 = d.N1, J = d.J;
-    T* su = sp + Nfp;
-    T* sv = su + Nfp;
-    T* sg = sv + Nfp;                             // [3 N1]
-    const int t = blockIdx.x, n = threadIdx.x;
-    const T* g = d.geo2 + (size_t)t * GEO2;
+    const int Nfp = d.Nfp, N1 = d.N1, J = d.J, Nf = 3 * d.N1;
+    const int W = max(Nfp, Nf);                   // thread slots per pair (3 N1 > Nfp for N <= 3)
+    const int PB = max(1, FACE2D_NT / W);
+    T* sD = reinterpret_cast<T*>(smem_raw);       // [2][Nfp(k)][Nfp(n)]
+    T* sL = sD + 2 * Nfp * Nfp;                   // [3 N1 (j)][Nfp(n)]
+    T* sp = sL + Nf * Nfp;                        // [PB][Nfp]
+    T* su = sp + PB * Nfp;
+    T* sv = su + PB * Nfp;
+    T* sg = sv + PB * Nfp;                        // [PB][3 N1]
+    const int tid = threadIdx.x;
+    for (int idx = tid; idx < 2 * Nfp * Nfp; idx += FACE2D_NT) {
+        const int a = idx / (Nfp * Nfp), r = idx - a * Nfp * Nfp, k = r / Nfp, n = r - k * Nfp;
+        sD[idx] = d.D2[(size_t)a * Nfp * Nfp + n * Nfp + k];
+    }
+    for (int idx = tid; idx < Nf * Nfp; idx += FACE2D_NT) {
+        const int j = idx / Nfp, n = idx - j * Nfp;
+        sL[idx] = d.L2[n * Nf + j];
+    }
+    const int pl = tid / W, n = tid - pl * W;
+    const bool active = pl < PB;
+    const int npairs = d.Tn * J, nchunk = (npairs + PB - 1) / PB;
     const T* fold = d.fa[src];
     T* fnew = d.fa[src ^ 1];
-    const size_t tstride = (size_t)J * 3 * Nfp;
-    const T Sown = (n < Nfp) ? d.S2[(size_t)t * Nfp + n] : T(0);
-    // face-node role of this thread (n < 3 N1)
-    int e = 0, m = 0, a = 0, nb = 0, bnode = 0;
-    T nxe = 0, nye = 0, Ae = 0, Be = 0, Sn = 0;
-    if (n < 3 * N1) {
-        e = n / N1; m = n - e * N1;
-        a = d.fmask2[n];
-        nb = d.nbr2[t * 3 + e];
-        bnode = d.nbrnode2[(t * 3 + e) * N1 + m];
-        nxe = g[4 + 2 * e]; nye = g[5 + 2 * e];
-        Ae = g[13 + e]; Be = g[16 + e];
-        if (nb >= 0) Sn = d.S2[(size_t)nb * Nfp + bnode];
-    }
-    for (int i = 0; i < J; ++i) {
-        const size_t o = (size_t)t * tstride + (size_t)i * 3 * Nfp;
+    T* mp = sp + pl * Nfp; T* mu = su + pl * Nfp; T* mv = sv + pl * Nfp; T* mg = sg + pl * Nf;
+    __syncthreads();
+    for (int chunk = blockIdx.x; chunk < nchunk; chunk += gridDim.x) {
+        const int pair = chunk * PB + pl;
+        const bool valid = active && pair < npairs;
+        const int t = valid ? pair / J : 0, i = valid ? pair - t * J : 0;
+        const size_t o = (size_t)pair * 3 * Nfp;
+        const T* g = d.geo2 + (size_t)t * GEO2;
         T ps = 0, u = 0, v = 0;
-        if (n < Nfp) {
+        if (valid && n < Nfp) {
             ps = fold[o + n]; u = fold[o + Nfp + n]; v = fold[o + 2 * Nfp + n];
-            sp[n] = ps + Sown; su[n] = u; sv[n] = v;
+            mp[n] = ps + d.S2[(size_t)t * Nfp + n]; mu[n] = u; mv[n] = v;
         }
         __syncthreads();
-        if (n < 3 * N1) {
-            const T pM = sp[a], unM = nxe * su[a] + nye * sv[a];
+        if (valid && n < Nf) {
+            // flux jump at edge node (e, m) of the triangle: neighbour triangle of the same domain face, or the
+            // ghost state (2 r^-, 0) behind a domain edge (qb2 from the edge closure)
+            const int e = n / N1, m = n - e * N1;
+            const int a = d.fmask2[n];
+            const int nb = d.nbr2[t * 3 + e];
+            const int bnode = d.nbrnode2[(t * 3 + e) * N1 + m];
+            const T nxe = g[4 + 2 * e], nye = g[5 + 2 * e];
+            const T pM = mp[a], unM = nxe * mu[a] + nye * mv[a];
             T pP, unP;
             if (nb >= 0) {
-                const size_t on = (size_t)nb * tstride + (size_t)i * 3 * Nfp;
-                pP = fold[on + bnode] + Sn;
+                const size_t on = ((size_t)nb * J + i) * 3 * Nfp;
+                pP = fold[on + bnode] + d.S2[(size_t)nb * Nfp + bnode];
                 unP = nxe * fold[on + Nfp + bnode] + nye * fold[on + 2 * Nfp + bnode];
             } else {
                 pP = T(2) * d.qb2[((size_t)(-1 - nb) * J + i) * N1 + bnode];
                 unP = 0;
             }
-            sg[n] = Ae * (unP - unM) - Be * (pP - pM);
+            mg[n] = g[13 + e] * (unP - unM) - g[16 + e] * (pP - pM);
         }
         __syncthreads();
-        if (n < Nfp) {
+        if (valid && n < Nfp) {
             T pr = 0, pss = 0, ur = 0, us = 0, vr = 0, vs = 0;
-            const T* Dr = d.D2 + (size_t)n * Nfp;
-            const T* Ds = d.D2 + (size_t)Nfp * Nfp + (size_t)n * Nfp;
+            const T* Dr = sD + n;
+            const T* Ds = sD + Nfp * Nfp + n;
             for (int k = 0; k < Nfp; ++k) {
-                const T a_ = Dr[k], b_ = Ds[k];
-                pr += a_ * sp[k]; pss += b_ * sp[k];
-                ur += a_ * su[k]; us += b_ * su[k];
-                vr += a_ * sv[k]; vs += b_ * sv[k];
+                const T a_ = Dr[k * Nfp], b_ = Ds[k * Nfp];
+                const T pk = mp[k], uk = mu[k], vk = mv[k];
+                pr += a_ * pk; pss += b_ * pk;
+                ur += a_ * uk; us += b_ * uk;
+                vr += a_ * vk; vs += b_ * vk;
             }
             // G2 = (r_xi, r_eta, s_xi, s_eta)
             const T dpx = g[0] * pr + g[2] * pss, dpy = g[1] * pr + g[3] * pss;
             const T div = g[0] * ur + g[2] * us + g[1] * vr + g[3] * vs;
             T lp = 0, lx = 0, ly = 0;
-            const T* L = d.L2 + (size_t)n * 3 * N1;
             for (int ee = 0; ee < 3; ++ee) {
                 T acc = 0;
-                for (int k = 0; k < N1; ++k) acc += L[ee * N1 + k] * sg[ee * N1 + k];
+                for (int k = 0; k < N1; ++k) acc += sL[(ee * N1 + k) * Nfp + n] * mg[ee * N1 + k];
                 const T fs = g[10 + ee];
                 lp += fs * acc; lx += fs * g[4 + 2 * ee] * acc; ly += fs * g[5 + 2 * ee] * acc;
             }
