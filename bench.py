@@ -148,17 +148,14 @@ def main():
         return run_reference(args)
 
     import torch
-    import torch.distributed as dist
     from paper_1610_05023_b200 import Solver
+    from paper_1610_05023_b200.replicas import Replicas
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    rep = Replicas.from_env("nccl")
+    rank, world, local = rep.rank, rep.world, rep.local
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     w = make_workload(args.workload, n=args.n)
     prec = args.precision
@@ -172,10 +169,7 @@ def main():
     t_setup = time.perf_counter() - t_setup
     nodes = s.K * s.Np
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    barrier = rep.barrier
 
     # ---- device-resident throughput
     s.step(args.warmup)
@@ -189,11 +183,7 @@ def main():
         ev1.record(s.stream)
     barrier()
     sampler.stop_flag = True
-    ms = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = rep.max_over_ranks(ev0.elapsed_time(ev1))
     value = world * nodes * args.steps / (ms * 1e-3)
 
     # ---- per-kernel device time (outside the timed region): the dominant kernel's roofline
@@ -237,11 +227,7 @@ def main():
     s.set_initial(*fields)
     s.step(args.steps)
     q, _, _ = s.get_fields(aux=False)
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = rep.max_over_ranks(time.perf_counter() - t0)
     h2d = 4 * nodes * (prec // 8)
     e2e = {"value": world * nodes * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d / args.steps,
            "d2h_bytes_per_step": h2d / args.steps, "seconds": e2e_s,
@@ -266,8 +252,7 @@ def main():
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
     if rank == 0:
         print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 if __name__ == "__main__":
