@@ -141,6 +141,7 @@ def main():
     ap.add_argument("--precision", type=int, default=64)
     ap.add_argument("--n", type=int, default=None, help="override hexes per side (debug only; invalidates the metric)")
     ap.add_argument("--impl", default="ours")
+    ap.add_argument("--kernel", type=int, default=0, help="dg_options.kernel (0 = the library's choice)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
@@ -160,7 +161,7 @@ def main():
     w = make_workload(args.workload, n=args.n)
     prec = args.precision
     t_setup = time.perf_counter()
-    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local)
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, kernel=args.kernel)
     x, y, z = s.get_nodes()
     cn = np.repeat(w.c[:, None], s.Np, axis=1)
     fields = [np.ascontiguousarray(f) for f in w.fields(x, y, z, cn, 1.0)]

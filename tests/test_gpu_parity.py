@@ -71,9 +71,10 @@ def test_J8_degree(N):
         _check(parity.compare(lib, ora), prec)
 
 
-@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (5, 1), (5, 2), (5, 3), (2, 2)])
+@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (4, 4), (5, 1), (5, 2), (5, 3), (5, 4), (2, 2)])
 def test_3d_kernel_variants(N, kernel):
-    """dg_options.kernel: 1 scalar FMA, 2 batch-synchronous DMMA, 3 warp-specialised DMMA -- the same numbers.
+    """dg_options.kernel: 1 scalar FMA, 2 batch-synchronous DMMA, 3 warp-specialised DMMA, 4 the same with the update in
+    its own warpgroup -- the same numbers.
     5^3 hexes = 750 tets: 93 batches of 8 + a ragged tail of 6, several batches per persistent CTA."""
     w = make_workload("cfg5", n=5, N=N, J=3, nsteps=12)
     lib, ora = parity.run_library(w, kernel=kernel), parity.run_oracle(w)
