@@ -215,12 +215,12 @@ def main():
                  "roof_ms": 1e3 * max(t_mem, t_alu), "frac_of_slower_roof": max(t_mem, t_alu) / (vol_ms * 1e-3),
                  "hbm": hbm, "alu": alu, "kernel_share_of_step": prof["vol3d"] / max(sum(prof.values()), 1e-12),
                  "per_kernel_ms_per_step": prof})
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")     # from the ncu --set full captures under profiles/
     if os.path.exists(traffic_file):
-        try:
-            roof["traffic"] = json.load(open(traffic_file)).get(f"{args.workload}_f{prec}")
-        except Exception:
-            pass
+        for ln in open(traffic_file).read().splitlines()[1:]:
+            cols = ln.split(",")
+            if cols and cols[0] == f"{args.workload}_f{prec}":
+                roof["traffic"] = float(cols[1])
 
     # ---- end to end through the C ABI with host buffers: H2D of the fields, the steps, D2H of the fields
     barrier()
