@@ -415,8 +415,9 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool con
 template <typename T>
 void launch_face2d(dg_solver* s, Dev<T>& d, int src, double a, double b) {
     const int Nf = 3 * d.N1, PB = std::max(1, FACE2D_NT / std::max(d.Nfp, Nf));
-    const size_t smem = sizeof(T) * (2 * d.Nfp * d.Nfp + Nf * d.Nfp + PB * (3 * d.Nfp + Nf));
-    const int nchunk = (d.Tn * d.J + PB - 1) / PB;
+    const size_t smem = sizeof(T) * (face2d_ops_elems(d.Nfp, d.N1) + (size_t)PB * (5 * d.Nfp + Nf) * FACE2D_SB);
+    const int nitems = d.Tn * ((d.J + FACE2D_SB - 1) / FACE2D_SB);
+    const int nchunk = (nitems + PB - 1) / PB;
     const int grid = std::max(1, std::min(nchunk, s->face_grid));
     k_face2d<T><<<grid, FACE2D_NT, smem, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
 }
@@ -717,6 +718,8 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
             int sms = 0;
             cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
             s->face_grid = sms * 8;
+            cu(cudaFuncSetAttribute(k_face2d<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024), "smem attr");
+            cu(cudaFuncSetAttribute(k_face2d<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024), "smem attr");
         }
         const size_t need = dry_bytes(s);
         if (opt && opt->workspace_dev) {

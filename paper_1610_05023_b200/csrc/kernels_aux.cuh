@@ -10,22 +10,58 @@ namespace dg {
 // 2D: the J face solvers (operators reused across sets, L631).
 // eq (31a-c): (1+c_i) dt p*_i + rho c^2 div_par U_i = 0 ; rho dt U_i + grad_par p_i = 0, p_i = p*_i + S.
 // ---------------------------------------------------------------------------------------------------
-// Threads <-> (pair, node), pair = (triangle t, set i): FACE2D_NT / max(Nfp, 3 N1) pairs per pass of a persistent CTA, the
-// operators D_r, D_s, LIFT2D staged once per CTA in shared memory (transposed: lanes <-> consecutive nodes).
+// Work item = (triangle t, group of FACE2D_SB = 4 consecutive sets i); thread <-> (item, node), FACE2D_NT /
+// max(Nfp, 3 N1) items per pass of a persistent CTA.  The operators D_r, D_s, LIFT2D are staged once per CTA in
+// shared memory (transposed: lanes <-> consecutive nodes) and every operator entry a thread fetches is used for the
+// four sets of its item (fields stored [node][set], one 32-byte broadcast load per field): 2 + 3 shared loads
+// per 16 FMA instead of 5 per 6, which is what moves the kernel from the shared-memory pipe (profiles/
+// r02_face2d_ncu.md: L1 data pipe 66 %, 657 us) to the FMA pipe.  The sets of one triangle also share its
+// geometry, its cached closure S and its neighbour lookups.
 constexpr int FACE2D_NT = 128;
+constexpr int FACE2D_SB = 4;
 
+template <typename T> __device__ __forceinline__ void ld4(const T* p, T (&v)[4]);
+template <> __device__ __forceinline__ void ld4<double>(const double* p, double (&v)[4]) {
+    const double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2);
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+}
+template <> __device__ __forceinline__ void ld4<float>(const float* p, float (&v)[4]) {
+    const float4 a = *reinterpret_cast<const float4*>(p);
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+}
+template <typename T> __device__ __forceinline__ void st4(T* p, const T (&v)[4]);
+template <> __device__ __forceinline__ void st4<double>(double* p, const double (&v)[4]) {
+    *reinterpret_cast<double2*>(p) = make_double2(v[0], v[1]);
+    *reinterpret_cast<double2*>(p + 2) = make_double2(v[2], v[3]);
+}
+template <> __device__ __forceinline__ void st4<float>(float* p, const float (&v)[4]) {
+    *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+}
+
+__host__ __device__ inline int face2d_ops_elems(int Nfp, int N1) {          // operators + 1/(1+c_i), padded to 4
+    return ((2 * Nfp * Nfp + 3 * N1 * Nfp + 3) / 4) * 4 + 16;
+}
+
+#ifndef FACE2D_MINB
+#define FACE2D_MINB 4
+#endif
 template <typename T>
-__global__ void __launch_bounds__(FACE2D_NT) k_face2d(Dev<T> d, int src, T rka, T rkb, T dt) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+__global__ void __launch_bounds__(FACE2D_NT, FACE2D_MINB) k_face2d(Dev<T> d, int src, T rka, T rkb, T dt) {
+    extern __shared__ __align__(32) unsigned char smem_raw[];
+    constexpr int SB = FACE2D_SB;
     const int Nfp = d.Nfp, N1 = d.N1, J = d.J, Nf = 3 * d.N1;
-    const int W = max(Nfp, Nf);                   // thread slots per pair (3 N1 > Nfp for N <= 3)
+    const int W = max(Nfp, Nf);                   // thread slots per item (3 N1 > Nfp for N <= 3)
     const int PB = max(1, FACE2D_NT / W);
+    const int NG = (J + SB - 1) / SB;             // set groups per triangle
     T* sD = reinterpret_cast<T*>(smem_raw);       // [2][Nfp(k)][Nfp(n)]
     T* sL = sD + 2 * Nfp * Nfp;                   // [3 N1 (j)][Nfp(n)]
-    T* sp = sL + Nf * Nfp;                        // [PB][Nfp]
-    T* su = sp + PB * Nfp;
-    T* sv = su + PB * Nfp;
-    T* sg = sv + PB * Nfp;                        // [PB][3 N1]
+    T* sIc = sD + face2d_ops_elems(Nfp, N1) - 16; // [J] 1 / (1 + c_i)   (eq (31a))
+    T* sp = sD + face2d_ops_elems(Nfp, N1);       // [PB][Nfp][SB]  p_i00 = p*_i + S   (eq (29))
+    T* sr = sp + PB * Nfp * SB;                   //                contravariant velocity U^r
+    T* ss = sr + PB * Nfp * SB;                   //                U^s
+    T* su = ss + PB * Nfp * SB;                   //                u, v (for the traces)
+    T* sv = su + PB * Nfp * SB;
+    T* sg = sv + PB * Nfp * SB;                   // [PB][3 N1][SB] flux jumps
     const int tid = threadIdx.x;
     for (int idx = tid; idx < 2 * Nfp * Nfp; idx += FACE2D_NT) {
         const int a = idx / (Nfp * Nfp), r = idx - a * Nfp * Nfp, k = r / Nfp, n = r - k * Nfp;
@@ -35,23 +71,51 @@ __global__ void __launch_bounds__(FACE2D_NT) k_face2d(Dev<T> d, int src, T rka, 
         const int j = idx / Nfp, n = idx - j * Nfp;
         sL[idx] = d.L2[n * Nf + j];
     }
+    for (int i = tid; i < 16; i += FACE2D_NT) sIc[i] = i < J ? T(1) / (T(1) + d.cn[i]) : T(0);
     const int pl = tid / W, n = tid - pl * W;
     const bool active = pl < PB;
-    const int npairs = d.Tn * J, nchunk = (npairs + PB - 1) / PB;
-    const T* fold = d.fa[src];
-    T* fnew = d.fa[src ^ 1];
-    T* mp = sp + pl * Nfp; T* mu = su + pl * Nfp; T* mv = sv + pl * Nfp; T* mg = sg + pl * Nf;
+    const int nitems = d.Tn * NG, nchunk = (nitems + PB - 1) / PB;
+    const T* __restrict__ fold = d.fa[src];
+    T* __restrict__ fnew = d.fa[src ^ 1];
+    T* mp = sp + pl * Nfp * SB; T* mr = sr + pl * Nfp * SB; T* ms = ss + pl * Nfp * SB;
+    T* mu = su + pl * Nfp * SB; T* mv = sv + pl * Nfp * SB; T* mg = sg + pl * Nf * SB;
     __syncthreads();
+    // fields of this thread's (item, node) for the current chunk; loaded one chunk ahead (global latency is the
+    // cost of this kernel: the same warps load, exchange through shared memory, gather and compute)
+    T ps[SB], u[SB], v[SB];
+    auto load_fields = [&](int chunk_, T (&a_)[SB], T (&b_)[SB], T (&c_)[SB]) {
+        const int item_ = chunk_ * PB + pl;
+        const bool ok_ = active && chunk_ < nchunk && item_ < nitems && n < Nfp;
+        const int t_ = ok_ ? item_ / NG : 0, i0_ = ok_ ? (item_ - t_ * NG) * SB : 0;
+        const size_t o_ = ((size_t)t_ * J + i0_) * 3 * Nfp + n;
+#pragma unroll
+        for (int q = 0; q < SB; ++q) {
+            const bool okq = ok_ && i0_ + q < J;
+            a_[q] = okq ? fold[o_ + (size_t)q * 3 * Nfp] : T(0);
+            b_[q] = okq ? fold[o_ + (size_t)q * 3 * Nfp + Nfp] : T(0);
+            c_[q] = okq ? fold[o_ + (size_t)q * 3 * Nfp + 2 * Nfp] : T(0);
+        }
+    };
+    load_fields(blockIdx.x, ps, u, v);
     for (int chunk = blockIdx.x; chunk < nchunk; chunk += gridDim.x) {
-        const int pair = chunk * PB + pl;
-        const bool valid = active && pair < npairs;
-        const int t = valid ? pair / J : 0, i = valid ? pair - t * J : 0;
-        const size_t o = (size_t)pair * 3 * Nfp;
-        const T* g = d.geo2 + (size_t)t * GEO2;
-        T ps = 0, u = 0, v = 0;
+        const int item = chunk * PB + pl;
+        const bool valid = active && item < nitems;
+        const int t = valid ? item / NG : 0, i0 = valid ? (item - t * NG) * SB : 0;
+        const int ns = min(SB, J - i0);
+        const size_t o = ((size_t)t * J + i0) * 3 * Nfp;          // set q of the item at o + q * 3 Nfp
+        const T* g = d.geo2 + (size_t)t * GEO2;                   // G2 = (r_xi, r_eta, s_xi, s_eta) | n[3][2] | ...
         if (valid && n < Nfp) {
-            ps = fold[o + n]; u = fold[o + Nfp + n]; v = fold[o + 2 * Nfp + n];
-            mp[n] = ps + d.S2[(size_t)t * Nfp + n]; mu[n] = u; mv[n] = v;
+            const T S = d.S2[(size_t)t * Nfp + n];
+            const T g0 = g[0], g1 = g[1], g2 = g[2], g3 = g[3];
+            T pp[SB], ur[SB], us[SB];
+#pragma unroll
+            for (int q = 0; q < SB; ++q) {
+                pp[q] = ps[q] + S;
+                ur[q] = g0 * u[q] + g1 * v[q];
+                us[q] = g2 * u[q] + g3 * v[q];
+            }
+            st4<T>(mp + n * SB, pp); st4<T>(mr + n * SB, ur); st4<T>(ms + n * SB, us);
+            st4<T>(mu + n * SB, u); st4<T>(mv + n * SB, v);
         }
         __syncthreads();
         if (valid && n < Nf) {
@@ -61,50 +125,92 @@ __global__ void __launch_bounds__(FACE2D_NT) k_face2d(Dev<T> d, int src, T rka, 
             const int a = d.fmask2[n];
             const int nb = d.nbr2[t * 3 + e];
             const int bnode = d.nbrnode2[(t * 3 + e) * N1 + m];
-            const T nxe = g[4 + 2 * e], nye = g[5 + 2 * e];
-            const T pM = mp[a], unM = nxe * mu[a] + nye * mv[a];
-            T pP, unP;
+            const T nxe = g[4 + 2 * e], nye = g[5 + 2 * e], Ae = g[13 + e], Be = g[16 + e];
+            T pM[SB], uM[SB], vM[SB], gj[SB];
+            ld4<T>(mp + a * SB, pM); ld4<T>(mu + a * SB, uM); ld4<T>(mv + a * SB, vM);
             if (nb >= 0) {
-                const size_t on = ((size_t)nb * J + i) * 3 * Nfp;
-                pP = fold[on + bnode] + d.S2[(size_t)nb * Nfp + bnode];
-                unP = nxe * fold[on + Nfp + bnode] + nye * fold[on + 2 * Nfp + bnode];
+                const T Sn = d.S2[(size_t)nb * Nfp + bnode];
+                const size_t on = ((size_t)nb * J + i0) * 3 * Nfp + bnode;
+#pragma unroll
+                for (int q = 0; q < SB; ++q) {
+                    const bool ok = q < ns;
+                    const T pP = (ok ? fold[on + (size_t)q * 3 * Nfp] : T(0)) + Sn;
+                    const T uP = ok ? fold[on + (size_t)q * 3 * Nfp + Nfp] : T(0);
+                    const T vP = ok ? fold[on + (size_t)q * 3 * Nfp + 2 * Nfp] : T(0);
+                    gj[q] = Ae * ((nxe * uP + nye * vP) - (nxe * uM[q] + nye * vM[q])) - Be * (pP - pM[q]);
+                }
             } else {
-                pP = T(2) * d.qb2[((size_t)(-1 - nb) * J + i) * N1 + bnode];
-                unP = 0;
+                const T* qb = d.qb2 + ((size_t)(-1 - nb) * J + i0) * N1 + bnode;
+#pragma unroll
+                for (int q = 0; q < SB; ++q) {
+                    const T pP = q < ns ? T(2) * qb[(size_t)q * N1] : T(0);
+                    gj[q] = Ae * (T(0) - (nxe * uM[q] + nye * vM[q])) - Be * (pP - pM[q]);
+                }
             }
-            mg[n] = g[13 + e] * (unP - unM) - g[16 + e] * (pP - pM);
+            st4<T>(mg + n * SB, gj);
         }
         __syncthreads();
+        T nps[SB], nu[SB], nv[SB];
+        load_fields(chunk + gridDim.x, nps, nu, nv);
         if (valid && n < Nfp) {
-            T pr = 0, pss = 0, ur = 0, us = 0, vr = 0, vs = 0;
+            T f0[SB], f1[SB], f2[SB];                             // res of this (item, node): loaded before the contraction
+#pragma unroll
+            for (int q = 0; q < SB; ++q) {
+                const size_t oq = o + (size_t)q * 3 * Nfp + n;
+                f0[q] = q < ns ? d.fres[oq] : T(0); f1[q] = q < ns ? d.fres[oq + Nfp] : T(0); f2[q] = q < ns ? d.fres[oq + 2 * Nfp] : T(0);
+            }
+            T pr[SB], pq[SB], dv[SB];
+#pragma unroll
+            for (int q = 0; q < SB; ++q) pr[q] = pq[q] = dv[q] = T(0);
             const T* Dr = sD + n;
             const T* Ds = sD + Nfp * Nfp + n;
             for (int k = 0; k < Nfp; ++k) {
                 const T a_ = Dr[k * Nfp], b_ = Ds[k * Nfp];
-                const T pk = mp[k], uk = mu[k], vk = mv[k];
-                pr += a_ * pk; pss += b_ * pk;
-                ur += a_ * uk; us += b_ * uk;
-                vr += a_ * vk; vs += b_ * vk;
+                T pk[SB], rk[SB], sk[SB];
+                ld4<T>(mp + k * SB, pk); ld4<T>(mr + k * SB, rk); ld4<T>(ms + k * SB, sk);
+#pragma unroll
+                for (int q = 0; q < SB; ++q) {
+                    pr[q] += a_ * pk[q]; pq[q] += b_ * pk[q];
+                    dv[q] += a_ * rk[q]; dv[q] += b_ * sk[q];
+                }
             }
-            // G2 = (r_xi, r_eta, s_xi, s_eta)
-            const T dpx = g[0] * pr + g[2] * pss, dpy = g[1] * pr + g[3] * pss;
-            const T div = g[0] * ur + g[2] * us + g[1] * vr + g[3] * vs;
-            T lp = 0, lx = 0, ly = 0;
+            T lp[SB], lx[SB], ly[SB];
+#pragma unroll
+            for (int q = 0; q < SB; ++q) lp[q] = lx[q] = ly[q] = T(0);
             for (int ee = 0; ee < 3; ++ee) {
-                T acc = 0;
-                for (int k = 0; k < N1; ++k) acc += sL[(ee * N1 + k) * Nfp + n] * mg[ee * N1 + k];
-                const T fs = g[10 + ee];
-                lp += fs * acc; lx += fs * g[4 + 2 * ee] * acc; ly += fs * g[5 + 2 * ee] * acc;
+                T acc[SB];
+#pragma unroll
+                for (int q = 0; q < SB; ++q) acc[q] = T(0);
+                for (int k = 0; k < N1; ++k) {
+                    const T l = sL[(ee * N1 + k) * Nfp + n];
+                    T gk[SB];
+                    ld4<T>(mg + (ee * N1 + k) * SB, gk);
+#pragma unroll
+                    for (int q = 0; q < SB; ++q) acc[q] += l * gk[q];
+                }
+                const T fs = g[10 + ee], fx = fs * g[4 + 2 * ee], fy = fs * g[5 + 2 * ee];
+#pragma unroll
+                for (int q = 0; q < SB; ++q) { lp[q] += fs * acc[q]; lx[q] += fx * acc[q]; ly[q] += fy * acc[q]; }
             }
+            const T g0 = g[0], g1 = g[1], g2 = g[2], g3 = g[3];
             const T rc2 = g[19], irho = g[20], cc = g[21];
-            const T rp = -rc2 * (div + lp) / (T(1) + d.cn[i]);
-            const T ru = -irho * dpx + cc * lx;
-            const T rv = -irho * dpy + cc * ly;
-            T r0 = d.fres[o + n], r1 = d.fres[o + Nfp + n], r2 = d.fres[o + 2 * Nfp + n];
-            r0 = rka * r0 + dt * rp; r1 = rka * r1 + dt * ru; r2 = rka * r2 + dt * rv;
-            d.fres[o + n] = r0; d.fres[o + Nfp + n] = r1; d.fres[o + 2 * Nfp + n] = r2;
-            fnew[o + n] = ps + rkb * r0; fnew[o + Nfp + n] = u + rkb * r1; fnew[o + 2 * Nfp + n] = v + rkb * r2;
+#pragma unroll
+            for (int q = 0; q < SB; ++q) {
+                if (q < ns) {
+                    const size_t oq = o + (size_t)q * 3 * Nfp + n;
+                    const T dpx = g0 * pr[q] + g2 * pq[q], dpy = g1 * pr[q] + g3 * pq[q];
+                    const T rp = -rc2 * (dv[q] + lp[q]) * sIc[i0 + q];
+                    const T ru = -irho * dpx + cc * lx[q];
+                    const T rv = -irho * dpy + cc * ly[q];
+                    T r0 = f0[q], r1 = f1[q], r2 = f2[q];
+                    r0 = rka * r0 + dt * rp; r1 = rka * r1 + dt * ru; r2 = rka * r2 + dt * rv;
+                    d.fres[oq] = r0; d.fres[oq + Nfp] = r1; d.fres[oq + 2 * Nfp] = r2;
+                    fnew[oq] = ps[q] + rkb * r0; fnew[oq + Nfp] = u[q] + rkb * r1; fnew[oq + 2 * Nfp] = v[q] + rkb * r2;
+                }
+            }
         }
+#pragma unroll
+        for (int q = 0; q < SB; ++q) { ps[q] = nps[q]; u[q] = nu[q]; v[q] = nv[q]; }
         __syncthreads();
     }
 }
