@@ -18,6 +18,7 @@
 #include "kernel_vol3d_mma.cuh"
 #include "kernel_vol3d_ws.cuh"
 #include "kernel_vol3d_ws2.cuh"
+#include "kernel_vol3d_tf32.cuh"
 #include "mesh.hpp"
 
 namespace {
@@ -79,7 +80,8 @@ struct dg_solver {
     bool mma3 = false;              // the tensor-pipe 3D kernel is in use
     bool ws3 = false;               // ... in its warp-specialised form (kernel_vol3d_ws.cuh)
     bool ws4 = false;               // ... with the update in its own warpgroup (kernel_vol3d_ws2.cuh); implies ws3
-    const double* geox3 = nullptr;  // [Kp][GX3] per-tet record of the warp-specialised kernel (dt folded in)
+    const void* geox3 = nullptr;    // [Kp][GX3] per-tet record of the warp-specialised kernels (dt folded in), fp64 or fp32
+    bool tf3 = false;               // fp32: the 3xTF32 tensor-core 3D kernel is in use (kernel_vol3d_tf32.cuh)
     bool use_graph = true;
     cudaGraphExec_t graph[2] = {nullptr, nullptr};
     std::vector<double> rho, c;
@@ -133,7 +135,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.N = m.N; d.J = J; d.K = K; d.Tn = Tn; d.E = E; d.C = C; d.Np = Np; d.Nfp = Nfp; d.N1 = N1;
     d.invM = T(1.0 / (2 * J + 1));
     // ---- 3D state
-    const size_t Kp = ((size_t)K + 7) / 8 * 8;     // the tensor-pipe kernel reads whole batches of 8 elements
+    const size_t Kp = ((size_t)K + 15) / 16 * 16;  // the tensor-pipe kernels read whole batches of 8 (fp64) / 16 (fp32) elements
     const size_t n3 = Kp * Np * 4;
     d.q[0] = U.zeros(n3); d.q[1] = U.zeros(n3); d.res = U.zeros(n3);
     std::vector<double> geo, dt3, lt3;
@@ -172,7 +174,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
         fm3.assign(m.r3.Fmask.begin(), m.r3.Fmask.end());
     }
     d.geo3 = U.real(geo, Kp * GEO3);
-    if (s->ws3) {
+    if (s->ws3 || s->tf3) {
         // record of kernel_vol3d_ws.cuh: G | dt rho c^2, dt/rho, dt c | (Fs n, A)_f | B_f | Fs_f
         std::vector<double> gx;
         if (!A.dry) {
@@ -191,7 +193,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
                 }
             }
         }
-        s->geox3 = (const double*)U.real(gx, Kp * GX3);
+        s->geox3 = U.real(gx, Kp * GX3);
     }
     d.nbr3 = U.template ints<int>(m.nbr3, (size_t)K * 4);
     d.finfo3 = U.template ints<uint32_t>(finfo, K);
@@ -349,7 +351,7 @@ void launch_vol3d_ws_cfg(dg_solver* s, Dev<double>& d, int src, double a, double
         s->smem3 = Cfg::smem_bytes;
         return;
     }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, s->geox3, src, a, b);
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const double*)s->geox3, src, a, b);
 }
 
 template <int N>
@@ -365,7 +367,7 @@ void launch_vol3d_ws2_cfg(dg_solver* s, Dev<double>& d, int src, double a, doubl
         s->smem3 = Cfg::smem_bytes;
         return;
     }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, s->geox3, src, a, b);
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const double*)s->geox3, src, a, b);
 }
 
 void launch_vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
@@ -393,9 +395,39 @@ void launch_vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b,
     }
 }
 
+template <int N>
+void launch_vol3d_tf32_cfg(dg_solver* s, Dev<float>& d, int src, double a, double b, bool configure) {
+    using Cfg = TfCfg<N>;
+    auto kern = k_vol3d_tf32<N>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int sms = 0;
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
+        s->grid3 = std::max(1, std::min(nbatch, sms));       // one persistent CTA per SM (it owns the register file)
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const float*)s->geox3, src, (float)a, (float)b);
+}
+
+constexpr int TF32_MIN_N = 3, TF32_MAX_N = 5;
+
+void launch_vol3d_tf32(dg_solver* s, Dev<float>& d, int src, double a, double b, bool configure) {
+    switch (s->N) {
+        case 3: return launch_vol3d_tf32_cfg<3>(s, d, src, a, b, configure);
+        case 4: return launch_vol3d_tf32_cfg<4>(s, d, src, a, b, configure);
+        case 5: return launch_vol3d_tf32_cfg<5>(s, d, src, a, b, configure);
+        default: throw std::runtime_error("EINVAL: the fp32 tensor-core kernel covers N = 3..5");
+    }
+}
+
 template <typename T>
 void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
     constexpr int mx = OpsFit<T>::maxN;
+    if constexpr (std::is_same<T, float>::value) {
+        if (s->tf3) return launch_vol3d_tf32(s, d, src, a, b, configure);
+    }
     if constexpr (std::is_same<T, double>::value) {
         if (s->mma3) return launch_vol3d_mma(s, d, src, a, b, configure);
     }
@@ -667,6 +699,7 @@ int dg_workspace_bytes(const dg_mesh* mesh, int N, int J, int precision, uint64_
         dg_solver s;
         s.N = N; s.J = J; s.precision = precision;
         s.ws3 = precision == 64 && N >= 4 && N <= 5;           // upper bound: covers every dg_options.kernel choice
+        s.tf3 = precision == 32 && N >= TF32_MIN_N && N <= TF32_MAX_N;
         s.m.N = N; s.m.K = mesh->ntets; s.m.C = 8;
         quick_counts(mesh, s.m.T, s.m.E);
         s.m.Np = (N + 1) * (N + 2) * (N + 3) / 6; s.m.Nfp = (N + 1) * (N + 2) / 2; s.m.N1 = N + 1;
@@ -690,13 +723,16 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
         s->use_graph = opt ? opt->use_graph != 0 : true;
         s->kernel = opt ? opt->kernel : 0;
-        if (s->kernel < 0 || s->kernel > 4) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..4");
-        if (s->kernel >= 3 && (precision != 64 || N < 4 || N > 5))
+        if (s->kernel < 0 || s->kernel > 5) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..5");
+        if (s->kernel == 5 && (precision != 32 || N < TF32_MIN_N || N > TF32_MAX_N))
+            throw std::runtime_error("EINVAL: the fp32 tensor-core kernel (kernel = 5) covers fp32, N = 3..5");
+        if ((s->kernel == 3 || s->kernel == 4) && (precision != 64 || N < 4 || N > 5))
             throw std::runtime_error("EINVAL: the warp-specialised kernels (kernel = 3, 4) cover fp64, N = 4, 5");
         if (s->kernel == 2 && (precision != 64 || N > MMA_MAX_N))
             throw std::runtime_error("EINVAL: the tensor-pipe kernel (kernel = 2) covers fp64, N = 1..5");
         if (mesh->ntets > CONN_MAX_ID) throw std::runtime_error("EINVAL: more than 2^26 - 1 tetrahedra");
         s->mma3 = precision == 64 && N <= MMA_MAX_N && s->kernel != 1;
+        s->tf3 = precision == 32 && N >= TF32_MIN_N && N <= TF32_MAX_N && (s->kernel == 0 || s->kernel == 5);
         s->ws4 = s->mma3 && s->kernel == 4;
         s->ws3 = s->mma3 && (s->ws4 || s->kernel == 3 || (s->kernel == 0 && N == 5));
         if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured

@@ -81,6 +81,20 @@ def test_3d_kernel_variants(N, kernel):
     _check(parity.compare(lib, ora), 64)
 
 
+@pytest.mark.parametrize("N,kernel", [(3, 5), (4, 5), (5, 5), (3, 1), (5, 1), (5, 0)])
+def test_3d_kernel_variants_fp32(N, kernel):
+    """fp32: 1 scalar FMA, 5 tensor cores with 3xTF32 error compensation (the default for N = 3..5) -- both inside the
+    fp32 tolerance, and the compensated tensor-core result no worse than 4x the FMA kernel's error.
+    750 tets = 46 batches of 16 + a ragged tail of 14."""
+    w = make_workload("cfg5", n=5, N=N, J=3, nsteps=12)
+    ora = parity.run_oracle(w)
+    err = parity.compare(parity.run_library(w, precision=32, kernel=kernel), ora)
+    _check(err, 32)
+    if kernel == 5:
+        ref = parity.compare(parity.run_library(w, precision=32, kernel=1), ora)
+        assert err["p"] <= 4 * ref["p"] + 1e-7 and err["u"] <= 4 * ref["u"] + 1e-7, (err, ref)
+
+
 def test_edge_cases():
     """Smallest mesh (one hex, 6 tets: every tet touches the boundary), J=1, J=12 (maximum), graph off,
     negatively oriented input cells, zero initial data, nsteps=0."""
