@@ -243,46 +243,65 @@ k_vol3d_tf32(Dev<float> d, const float* __restrict__ geox, int src, float rka, f
         mbar_wait(&ready[o], (it >> 1) & 1);
         mbar_wait(&full[s], (it / NS) & 1);                  // already complete: makes the async-proxy writes visible here
         // ---- contractions (eq (41)): accumulators [element g / g+8][node 8w+2t / +1]
-        float cpr[4] = {0, 0, 0, 0}, cps[4] = {0, 0, 0, 0}, cpt[4] = {0, 0, 0, 0}, cdv[4] = {0, 0, 0, 0};
+        // Issue order: the three MMAs of one product (lo*hi, hi*lo, hi*hi) hit the same accumulator, so they are
+        // issued as three PASSES over six (D part) or four (LIFT part) independent accumulators -- a dependent
+        // HMMA is then 6 (4) issue slots away and the tensor pipe never waits for its own result.
+        float cpr[4] = {0, 0, 0, 0}, cps[4] = {0, 0, 0, 0}, cpt[4] = {0, 0, 0, 0};
+        float cvr[4] = {0, 0, 0, 0}, cvs[4] = {0, 0, 0, 0}, cvt[4] = {0, 0, 0, 0};
         float cl[4][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
         {
             // A fragment of k-step s_: rows (elements) g, g+8; columns (k) 8 s_ + t, + 4
             const float* ap = sB + t * XS + g;
+            auto load = [&](const float* r0, uint32_t (&ah)[4], uint32_t (&al)[4]) {
+                const float x0 = r0[0], x1 = r0[8], x2 = r0[4 * XS], x3 = r0[4 * XS + 8];
+                split_tf32(x0, ah[0], al[0]);
+                split_tf32(x1, ah[1], al[1]);
+                split_tf32(x2, ah[2], al[2]);
+                split_tf32(x3, ah[3], al[3]);
+            };
 #pragma unroll
             for (int s_ = 0; s_ < KD; ++s_) {
-                uint32_t ah[4], al[4];
-                auto load = [&](const float* base) {
-                    const float* r0 = base + (8 * s_) * XS;
-                    split_tf32(r0[0], ah[0], al[0]);
-                    split_tf32(r0[8], ah[1], al[1]);
-                    split_tf32(r0[4 * XS], ah[2], al[2]);
-                    split_tf32(r0[4 * XS + 8], ah[3], al[3]);
-                };
-                load(ap);
-                mma_3x(cpr, ah, al, Brh[s_], Brl[s_]);
-                mma_3x(cps, ah, al, Bsh[s_], Bsl[s_]);
-                mma_3x(cpt, ah, al, Bth[s_], Btl[s_]);
-                load(ap + KPD * XS);
-                mma_3x(cdv, ah, al, Brh[s_], Brl[s_]);
-                load(ap + 2 * KPD * XS);
-                mma_3x(cdv, ah, al, Bsh[s_], Bsl[s_]);
-                load(ap + 3 * KPD * XS);
-                mma_3x(cdv, ah, al, Bth[s_], Btl[s_]);
+                uint32_t ph[4], pl[4], rh[4], rl[4], sh[4], sl[4], th[4], tl[4];
+                load(ap + (8 * s_) * XS, ph, pl);
+                load(ap + (KPD + 8 * s_) * XS, rh, rl);
+                load(ap + (2 * KPD + 8 * s_) * XS, sh, sl);
+                load(ap + (3 * KPD + 8 * s_) * XS, th, tl);
+                mma_tf32(cpr, pl, Brh[s_][0], Brh[s_][1]);
+                mma_tf32(cps, pl, Bsh[s_][0], Bsh[s_][1]);
+                mma_tf32(cpt, pl, Bth[s_][0], Bth[s_][1]);
+                mma_tf32(cvr, rl, Brh[s_][0], Brh[s_][1]);
+                mma_tf32(cvs, sl, Bsh[s_][0], Bsh[s_][1]);
+                mma_tf32(cvt, tl, Bth[s_][0], Bth[s_][1]);
+                mma_tf32(cpr, ph, Brl[s_][0], Brl[s_][1]);
+                mma_tf32(cps, ph, Bsl[s_][0], Bsl[s_][1]);
+                mma_tf32(cpt, ph, Btl[s_][0], Btl[s_][1]);
+                mma_tf32(cvr, rh, Brl[s_][0], Brl[s_][1]);
+                mma_tf32(cvs, sh, Bsl[s_][0], Bsl[s_][1]);
+                mma_tf32(cvt, th, Btl[s_][0], Btl[s_][1]);
+                mma_tf32(cpr, ph, Brh[s_][0], Brh[s_][1]);
+                mma_tf32(cps, ph, Bsh[s_][0], Bsh[s_][1]);
+                mma_tf32(cpt, ph, Bth[s_][0], Bth[s_][1]);
+                mma_tf32(cvr, rh, Brh[s_][0], Brh[s_][1]);
+                mma_tf32(cvs, sh, Bsh[s_][0], Bsh[s_][1]);
+                mma_tf32(cvt, th, Bth[s_][0], Bth[s_][1]);
             }
             const float* gp = ap + 4 * KPD * XS;
 #pragma unroll
-            for (int f = 0; f < 4; ++f)
+            for (int s_ = 0; s_ < KL; ++s_) {
+                uint32_t fh[4][4], fl[4][4];
 #pragma unroll
-                for (int s_ = 0; s_ < KL; ++s_) {
-                    uint32_t ah[4], al[4];
-                    const float* r0 = gp + (f * KPL + 8 * s_) * XS;
-                    split_tf32(r0[0], ah[0], al[0]);
-                    split_tf32(r0[8], ah[1], al[1]);
-                    split_tf32(r0[4 * XS], ah[2], al[2]);
-                    split_tf32(r0[4 * XS + 8], ah[3], al[3]);
-                    mma_3x(cl[f], ah, al, BLh[f][s_], BLl[f][s_]);
-                }
+                for (int f = 0; f < 4; ++f) load(gp + (f * KPL + 8 * s_) * XS, fh[f], fl[f]);
+#pragma unroll
+                for (int f = 0; f < 4; ++f) mma_tf32(cl[f], fl[f], BLh[f][s_][0], BLh[f][s_][1]);
+#pragma unroll
+                for (int f = 0; f < 4; ++f) mma_tf32(cl[f], fh[f], BLl[f][s_][0], BLl[f][s_][1]);
+#pragma unroll
+                for (int f = 0; f < 4; ++f) mma_tf32(cl[f], fh[f], BLh[f][s_][0], BLh[f][s_][1]);
+            }
         }
+        float cdv[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) cdv[i] = (cvr[i] + cvs[i]) + cvt[i];
         __syncwarp();
         if (lane == 0) mbar_arrive(&opfree[o]);
         // ---- right-hand side and LSRK update (eq (41)-(43)); dt is folded into the record.
