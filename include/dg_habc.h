@@ -59,8 +59,8 @@ typedef struct {
     int32_t kernel;           /* 3D kernel: 0 = the library's choice; 1 = scalar-FMA kernel (any N, fp64/fp32);
                                  2 = fp64 tensor-pipe (DMMA) kernel, N <= 5; 3 = its warp-specialised form, N = 4, 5
                                  (the choice at N = 5); 4 = experimental variant of 3 with the update in helper
-                                 warps; 5 = fp32 tensor-core kernel (3xTF32, fp32-accurate), N = 3..5 (the choice
-                                 there).  A kernel that does not cover (N, precision) gives DG_EINVAL */
+                                 warps; 6 = experimental variant of 3 with a software-pipelined MMA loop;
+                                 5 = fp32 tensor-core kernel (3xTF32, fp32-accurate), N = 3..5 (the choice there).  A kernel that does not cover (N, precision) gives DG_EINVAL */
 } dg_options;
 
 typedef struct {

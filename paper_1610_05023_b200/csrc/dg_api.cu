@@ -18,6 +18,7 @@
 #include "kernel_vol3d_mma.cuh"
 #include "kernel_vol3d_ws.cuh"
 #include "kernel_vol3d_ws2.cuh"
+#include "kernel_vol3d_wsp.cuh"
 #include "kernel_vol3d_tf32.cuh"
 #include "mesh.hpp"
 
@@ -79,6 +80,7 @@ struct dg_solver {
     int kernel = 0;                 // dg_options.kernel as requested
     bool mma3 = false;              // the tensor-pipe 3D kernel is in use
     bool ws3 = false;               // ... in its warp-specialised form (kernel_vol3d_ws.cuh)
+    bool ws6 = false;               // ... with the software-pipelined MMA loop (kernel_vol3d_wsp.cuh); implies ws3
     bool ws4 = false;               // ... with the update in its own warpgroup (kernel_vol3d_ws2.cuh); implies ws3
     const void* geox3 = nullptr;    // [Kp][GX3] per-tet record of the warp-specialised kernels (dt folded in), fp64 or fp32
     bool tf3 = false;               // fp32: the 3xTF32 tensor-core 3D kernel is in use (kernel_vol3d_tf32.cuh)
@@ -370,7 +372,30 @@ void launch_vol3d_ws2_cfg(dg_solver* s, Dev<double>& d, int src, double a, doubl
     kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const double*)s->geox3, src, a, b);
 }
 
+template <int N>
+void launch_vol3d_wsp_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    using Cfg = WspCfg<N>;
+    auto kern = k_vol3d_wsp<N>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int sms = 0;
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
+        s->grid3 = std::max(1, std::min(nbatch, sms));       // one persistent CTA per SM (it owns the register file)
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const double*)s->geox3, src, a, b);
+}
+
 void launch_vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    if (s->ws6) {
+        switch (s->N) {
+            case 4: return launch_vol3d_wsp_cfg<4>(s, d, src, a, b, configure);
+            case 5: return launch_vol3d_wsp_cfg<5>(s, d, src, a, b, configure);
+            default: throw std::runtime_error("EINVAL: the warp-specialised kernels cover N = 4, 5");
+        }
+    }
     if (s->ws4) {
         switch (s->N) {
             case 4: return launch_vol3d_ws2_cfg<4>(s, d, src, a, b, configure);
@@ -723,18 +748,19 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
         s->use_graph = opt ? opt->use_graph != 0 : true;
         s->kernel = opt ? opt->kernel : 0;
-        if (s->kernel < 0 || s->kernel > 5) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..5");
+        if (s->kernel < 0 || s->kernel > 6) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..6");
         if (s->kernel == 5 && (precision != 32 || N < TF32_MIN_N || N > TF32_MAX_N))
             throw std::runtime_error("EINVAL: the fp32 tensor-core kernel (kernel = 5) covers fp32, N = 3..5");
-        if ((s->kernel == 3 || s->kernel == 4) && (precision != 64 || N < 4 || N > 5))
-            throw std::runtime_error("EINVAL: the warp-specialised kernels (kernel = 3, 4) cover fp64, N = 4, 5");
+        if ((s->kernel == 3 || s->kernel == 4 || s->kernel == 6) && (precision != 64 || N < 4 || N > 5))
+            throw std::runtime_error("EINVAL: the warp-specialised kernels (kernel = 3, 4, 6) cover fp64, N = 4, 5");
         if (s->kernel == 2 && (precision != 64 || N > MMA_MAX_N))
             throw std::runtime_error("EINVAL: the tensor-pipe kernel (kernel = 2) covers fp64, N = 1..5");
         if (mesh->ntets > CONN_MAX_ID) throw std::runtime_error("EINVAL: more than 2^26 - 1 tetrahedra");
         s->mma3 = precision == 64 && N <= MMA_MAX_N && s->kernel != 1;
         s->tf3 = precision == 32 && N >= TF32_MIN_N && N <= TF32_MAX_N && (s->kernel == 0 || s->kernel == 5);
         s->ws4 = s->mma3 && s->kernel == 4;
-        s->ws3 = s->mma3 && (s->ws4 || s->kernel == 3 || (s->kernel == 0 && N == 5));
+        s->ws6 = s->mma3 && s->kernel == 6;
+        s->ws3 = s->mma3 && (s->ws4 || s->ws6 || s->kernel == 3 || (s->kernel == 0 && N == 5));
         if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured
         s->rho.assign(rho, rho + mesh->ntets);
         s->c.assign(c, c + mesh->ntets);
