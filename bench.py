@@ -140,6 +140,8 @@ def main():
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--precision", type=int, default=64)
     ap.add_argument("--n", type=int, default=None, help="override hexes per side (debug only; invalidates the metric)")
+    ap.add_argument("--N", type=int, default=None, help="override the polynomial degree (degree sweep of configs[3])")
+    ap.add_argument("--J", type=int, default=None, help="override the HABC order (degree sweep of configs[3])")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--kernel", type=int, default=0, help="dg_options.kernel (0 = the library's choice)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -158,7 +160,7 @@ def main():
     rank, world, local = rep.rank, rep.world, rep.local
     torch.cuda.set_device(local)
 
-    w = make_workload(args.workload, n=args.n)
+    w = make_workload(args.workload, n=args.n, N=args.N, J=args.J)
     prec = args.precision
     t_setup = time.perf_counter()
     s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, kernel=args.kernel)
