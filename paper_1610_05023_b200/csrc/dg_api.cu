@@ -288,8 +288,15 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     const size_t e2 = (size_t)4 * J * J, c2 = (size_t)9 * J * J * J * J;
     d.cn = U.real(h.cn, J);
     d.Cij = U.real(h.Cij, (size_t)J * J);
-    d.Pe = U.real(h.Pe, e2);
-    d.Qe = U.real(h.Qe, e2);
+    auto transposed = [](const std::vector<double>& M, int n) {
+        std::vector<double> Tm(M.size());
+        if (M.size() != (size_t)n * n) return Tm;              // sizing pass: the coefficients are not built yet
+        for (int r = 0; r < n; ++r)
+            for (int k = 0; k < n; ++k) Tm[(size_t)k * n + r] = M[(size_t)r * n + k];
+        return Tm;
+    };
+    d.PeT = U.real(transposed(h.Pe, 2 * J), e2);
+    d.QeT = U.real(transposed(h.Qe, 2 * J), e2);
     d.Gc = U.real(h.Gc, c2);
     // fp64 scratch for exporting the physical auxiliary fields
     s->export_elems = n2 + n1;
@@ -487,11 +494,11 @@ void launch_closures(dg_solver* s, Dev<T>& d, int cur) {
     k_close_face<T><<<(nf + 255) / 256, 256, 0, s->stream>>>(d, cur);
     if (d.E > 0) {
         const int ne = d.E * d.N1;
-        k_close_edge<T><<<(ne + 63) / 64, 64, 0, s->stream>>>(d, cur);
+        k_close_edge<T><<<(ne + CLOSE_EDGE_WARPS - 1) / CLOSE_EDGE_WARPS, 32 * CLOSE_EDGE_WARPS, 0, s->stream>>>(d, cur);
     }
     if (d.C > 0) {
         const int JJ3 = 3 * d.J * d.J;
-        k_close_corner<T><<<d.C, std::min(1024, ((JJ3 + 31) / 32) * 32), sizeof(T) * JJ3, s->stream>>>(d, cur);
+        k_close_corner<T><<<d.C, 1024, sizeof(T) * JJ3, s->stream>>>(d, cur);
     }
 }
 
@@ -642,11 +649,11 @@ void profile_step(dg_solver* s, Dev<T>& d, double* ms) {
             }
             const int cur = src ^ 1;
             timed(3, [&] { k_close_face<T><<<(d.Tn * d.Nfp + 255) / 256, 256, 0, s->stream>>>(d, cur); });
-            if (d.E > 0) timed(4, [&] { k_close_edge<T><<<(d.E * d.N1 + 63) / 64, 64, 0, s->stream>>>(d, cur); });
+            if (d.E > 0) timed(4, [&] { k_close_edge<T><<<(d.E * d.N1 + CLOSE_EDGE_WARPS - 1) / CLOSE_EDGE_WARPS, 32 * CLOSE_EDGE_WARPS, 0, s->stream>>>(d, cur); });
             if (d.C > 0) {
                 const int JJ3 = 3 * d.J * d.J;
                 timed(5, [&] {
-                    k_close_corner<T><<<d.C, std::min(1024, ((JJ3 + 31) / 32) * 32), sizeof(T) * JJ3, s->stream>>>(d, cur);
+                    k_close_corner<T><<<d.C, 1024, sizeof(T) * JJ3, s->stream>>>(d, cur);
                 });
             }
         }

@@ -64,7 +64,7 @@ struct Dev {
     // ---- HABC algebra
     const T* cn;                     // [J]
     const T* Cij;                    // [J][J]  (1+c_i)/(1+c_i+c_j)
-    const T* Pe; const T* Qe;        // [2J][2J] edge: r^- = Pe b + Qe r^+
+    const T* PeT; const T* QeT;      // [2J][2J] edge: r^- = Pe b + Qe r^+, stored transposed ([k][r])
     const T* Gc;                     // [3J^2][3J^2] corner: r^- = Gc r^+
     T invM;                          // 1/(2J+1)
 };

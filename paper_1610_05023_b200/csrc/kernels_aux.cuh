@@ -305,54 +305,68 @@ __global__ void k_close_face(Dev<T> d, int cur) {
     d.S2[idx] = rp + rm;
 }
 
-// edge: r^+ of both faces' 2D fields across the edge, the 2J x 2J system (33a-b) through its inverse
+// edge: r^+ of both faces' 2D fields across the edge, the 2J x 2J system (33a-b) through its inverse.
+// One WARP per edge node, lane k <-> unknown k of (r^{-a}_j ; r^{-b}_i): every lane gathers its own r^+ and
+// right-hand side b, the vectors are exchanged through shared memory and lane r takes row r of the inverse
+// (stored transposed: coalesced).  The first version ran one THREAD per node (~600 dependent loads, 60 us of
+// pure latency whatever the mesh size).
+constexpr int CLOSE_EDGE_WARPS = 4;
 template <typename T>
-__global__ void k_close_edge(Dev<T> d, int cur) {
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    const int J = d.J, N1 = d.N1, Nfp = d.Nfp;
-    if (idx >= d.E * N1) return;
-    const int ell = idx / N1, m = idx - ell * N1;
-    T b[2 * JMAX], rp[2 * JMAX];
-    // side 0 = face A supplies r^{+b}_i (stored at J+i), side 1 = face B supplies r^{+a}_j (stored at j)
-    for (int side = 0; side < 2; ++side) {
+__global__ void __launch_bounds__(32 * CLOSE_EDGE_WARPS) k_close_edge(Dev<T> d, int cur) {
+    __shared__ T sb[CLOSE_EDGE_WARPS][2 * JMAX], srp[CLOSE_EDGE_WARPS][2 * JMAX];
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int node = blockIdx.x * CLOSE_EDGE_WARPS + wl;
+    const int J = d.J, N1 = d.N1, Nfp = d.Nfp, J2 = 2 * J;
+    if (node >= d.E * N1) return;
+    const int ell = node / N1, m = node - ell * N1;
+    T rpk = 0;
+    if (lane < J2) {
+        // unknown k < J: r^{-a}_j, its r^{+a}_j comes from face B (side 1); k >= J: r^{-b}_i, r^{+b}_i from face A (side 0)
+        const int side = lane < J ? 1 : 0, sidx = lane < J ? lane : lane - J;
         const int t = d.lin_tri[ell * 2 + side];
         const int a = d.lin_trinode[(ell * 2 + side) * N1 + m];
         const T S = d.S2[(size_t)t * Nfp + a];
         const T Z = d.geo2[(size_t)t * GEO2 + 22];
         const int slot = d.lin_slot[ell * 2 + side];
         const T sg = T(d.lin_osign[ell * 2 + side]);
-        const T* f = d.fa[cur] + (size_t)t * J * 3 * Nfp;
-        for (int i = 0; i < J; ++i) {
-            const T p = f[(size_t)i * 3 * Nfp + a] + S;
-            const T u = sg * f[(size_t)i * 3 * Nfp + (1 + slot) * Nfp + a];
-            rp[(side == 0 ? J : 0) + i] = T(0.5) * (p + Z * u);
+        const T* f = d.fa[cur] + ((size_t)t * J + sidx) * 3 * Nfp;
+        const T p = f[a] + S;
+        const T u = sg * f[(1 + slot) * Nfp + a];
+        rpk = T(0.5) * (p + Z * u);
+        // b^a_j = sum_i c_i p*_ij ; b^b_i = sum_j c_j p*_ij
+        const T* ea = d.ea[cur] + (size_t)ell * J * J * 2 * N1 + m;
+        T bk = 0;
+        for (int q = 0; q < J; ++q) {
+            const int ij = lane < J ? q * J + sidx : sidx * J + q;
+            bk += d.cn[q] * ea[(size_t)ij * 2 * N1];
         }
+        sb[wl][lane] = bk;
+        srp[wl][lane] = rpk;
     }
-    const T* ea = d.ea[cur] + (size_t)ell * J * J * 2 * N1 + m;
-    for (int k = 0; k < 2 * J; ++k) b[k] = 0;
-    for (int i = 0; i < J; ++i)
-        for (int j = 0; j < J; ++j) {
-            const T ps = ea[(size_t)(i * J + j) * 2 * N1];
-            b[j] += d.cn[i] * ps;            // b^a_j = sum_i c_i p*_ij
-            b[J + i] += d.cn[j] * ps;        // b^b_i = sum_j c_j p*_ij
+    __syncwarp();
+    if (lane < J2) {
+        T acc0 = 0, acc1 = 0;
+        for (int k = 0; k < J2; ++k) {
+            acc0 += d.PeT[k * J2 + lane] * sb[wl][k];
+            acc1 += d.QeT[k * J2 + lane] * srp[wl][k];
         }
-    for (int r = 0; r < 2 * J; ++r) {
-        T acc = 0;
-        for (int k = 0; k < 2 * J; ++k) acc += d.Pe[r * 2 * J + k] * b[k] + d.Qe[r * 2 * J + k] * rp[k];
+        const T acc = acc0 + acc1;
         // r < J: r^{-a}_j (for face B's fields, side 1); r >= J: r^{-b}_i (for face A's fields, side 0)
-        const int side = r < J ? 1 : 0, s = r < J ? r : r - J;
-        d.qb2[(((size_t)ell * 2 + side) * J + s) * N1 + m] = acc;
-        d.S1[(((size_t)ell * 2 + (r < J ? 0 : 1)) * J + s) * N1 + m] = acc + rp[r];
+        const int r = lane, side = r < J ? 1 : 0, sidx = r < J ? r : r - J;
+        d.qb2[(((size_t)ell * 2 + side) * J + sidx) * N1 + m] = acc;
+        d.S1[(((size_t)ell * 2 + (r < J ? 0 : 1)) * J + sidx) * N1 + m] = acc + rpk;
     }
 }
 
-// corner: r^+ of the three edges' 1D fields at the corner, the 3J^2 system (35a-c) through Gc = L^-1 T
+// corner: r^+ of the three edges' 1D fields at the corner, the 3J^2 system (35a-c) through Gc = L^-1 T.
+// One CTA per corner; one WARP per row of Gc at a time, lanes across the columns (coalesced row reads, all loads
+// independent), shuffle reduction.
 template <typename T>
 __global__ void k_close_corner(Dev<T> d, int cur) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* srp = reinterpret_cast<T*>(smem_raw);      // [3 J^2]
-    const int J = d.J, JJ = J * J, N1 = d.N1, c = blockIdx.x;
-    for (int r = threadIdx.x; r < 3 * JJ; r += blockDim.x) {
+    const int J = d.J, JJ = J * J, N1 = d.N1, c = blockIdx.x, n3 = 3 * JJ;
+    for (int r = threadIdx.x; r < n3; r += blockDim.x) {
         const int ax = r / JJ, ij = r - ax * JJ;
         const int ell = d.cor_line[c * 3 + ax];
         const int node = d.cor_end[c * 3 + ax] ? N1 - 1 : 0;
@@ -362,11 +376,14 @@ __global__ void k_close_corner(Dev<T> d, int cur) {
         srp[r] = T(0.5) * (p + Z * T(d.cor_sign[c * 3 + ax]) * w);
     }
     __syncthreads();
-    for (int r = threadIdx.x; r < 3 * JJ; r += blockDim.x) {
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int r = wl; r < n3; r += nw) {
+        const T* row = d.Gc + (size_t)r * n3;
         T acc = 0;
-        const T* row = d.Gc + (size_t)r * 3 * JJ;
-        for (int k = 0; k < 3 * JJ; ++k) acc += row[k] * srp[k];
-        d.qb1[(size_t)(c * 3 + r / JJ) * JJ + (r % JJ)] = acc;
+        for (int k = lane; k < n3; k += 32) acc += row[k] * srp[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) d.qb1[(size_t)(c * 3 + r / JJ) * JJ + (r % JJ)] = acc;
     }
 }
 
