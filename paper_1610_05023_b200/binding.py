@@ -141,8 +141,12 @@ class Solver:
     def step(self, nsteps: int = 1):
         _check(lib().dg_step(self._h, int(nsteps)))
 
-    def get_fields(self, aux: bool = True):
-        q = np.empty((4, self.K, self.Np))
+    def get_fields(self, aux: bool = True, out=None):
+        """(q [4,K,Np], face_aux, edge_aux).  `out`: optional preallocated float64 C-contiguous [4,K,Np] array for q
+        (e.g. backed by pinned host memory) -- written in place and returned."""
+        q = np.empty((4, self.K, self.Np)) if out is None else out
+        if q.dtype != np.float64 or q.shape != (4, self.K, self.Np) or not q.flags["C_CONTIGUOUS"]:
+            raise DgError("get_fields(out=...): need a C-contiguous float64 array of shape (4, K, Np)")
         fa = np.zeros((self.T, self.J, 3, self.Nfp)) if aux else None
         ea = np.zeros((self.E, self.J * self.J, 2, self.N + 1)) if aux else None
         _check(lib().dg_get_fields(self._h, _dp(q[0]), _dp(q[1]), _dp(q[2]), _dp(q[3]), _dp(fa), _dp(ea)))

@@ -576,11 +576,15 @@ void check_args(const dg_mesh* mesh, int N, int J, int precision) {
 template <typename T>
 void upload_initial(dg_solver* s, Dev<T>& d, const double* p, const double* u, const double* v, const double* w) {
     const size_t n = (size_t)d.K * d.Np;
-    std::vector<T> h(n * 4);
-    for (size_t i = 0; i < n; ++i) {
-        h[i * 4] = (T)p[i]; h[i * 4 + 1] = (T)u[i]; h[i * 4 + 2] = (T)v[i]; h[i * 4 + 3] = (T)w[i];
+    // each fp64 field goes to the device as it is (q[1] is free here and serves as the staging area: it holds
+    // 4 n values of T >= n doubles) and is converted / interleaved into q[0] by a kernel
+    const double* fields[4] = {p, u, v, w};
+    double* stage = reinterpret_cast<double*>(d.q[1]);
+    for (int f = 0; f < 4; ++f) {
+        cu(cudaMemcpyAsync(stage, fields[f], sizeof(double) * n, cudaMemcpyHostToDevice, s->stream), "upload field");
+        k_pack_field<T><<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(stage, d.q[0], f, n);
     }
-    cu(cudaMemcpyAsync(d.q[0], h.data(), sizeof(T) * h.size(), cudaMemcpyHostToDevice, s->stream), "upload q");
+    cu(cudaGetLastError(), "pack launch");
     cu(cudaMemsetAsync(d.q[1], 0, sizeof(T) * n * 4, s->stream), "memset");
     cu(cudaMemsetAsync(d.res, 0, sizeof(T) * n * 4, s->stream), "memset");
     const size_t n2 = (size_t)d.Tn * d.J * 3 * d.Nfp, n1 = (size_t)d.E * d.J * d.J * 2 * d.N1;
@@ -598,16 +602,16 @@ void upload_initial(dg_solver* s, Dev<T>& d, const double* p, const double* u, c
 template <typename T>
 void download_fields(dg_solver* s, Dev<T>& d, double* p, double* u, double* v, double* w, double* fa, double* ea) {
     const size_t n = (size_t)d.K * d.Np;
-    if (p || u || v || w) {
-        std::vector<T> h(n * 4);
-        cu(cudaMemcpyAsync(h.data(), d.q[s->cur], sizeof(T) * h.size(), cudaMemcpyDeviceToHost, s->stream), "download q");
-        cu(cudaStreamSynchronize(s->stream), "sync");
-        for (size_t i = 0; i < n; ++i) {
-            if (p) p[i] = (double)h[i * 4];
-            if (u) u[i] = (double)h[i * 4 + 1];
-            if (v) v[i] = (double)h[i * 4 + 2];
-            if (w) w[i] = (double)h[i * 4 + 3];
+    {
+        // one field at a time through the buffer the next stage will overwrite anyway (q[cur ^ 1])
+        double* out[4] = {p, u, v, w};
+        double* stage = reinterpret_cast<double*>(d.q[s->cur ^ 1]);
+        for (int f = 0; f < 4; ++f) {
+            if (!out[f]) continue;
+            k_unpack_field<T><<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(d.q[s->cur], stage, f, n);
+            cu(cudaMemcpyAsync(out[f], stage, sizeof(double) * n, cudaMemcpyDeviceToHost, s->stream), "download field");
         }
+        cu(cudaGetLastError(), "unpack launch");
     }
     const size_t n2 = (size_t)d.Tn * d.J * 3 * d.Nfp, n1 = (size_t)d.E * d.J * d.J * 2 * d.N1;
     if ((fa || ea) && n2 + n1 > 0) {

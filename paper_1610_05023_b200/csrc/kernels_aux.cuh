@@ -387,6 +387,18 @@ __global__ void k_close_corner(Dev<T> d, int cur) {
     }
 }
 
+// dg_set_initial / dg_get_fields: interface arrays are fp64 [K][Np] per field; the device state is [K][Np][4] of T
+template <typename T>
+__global__ void k_pack_field(const double* __restrict__ stage, T* __restrict__ q, int fld, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) q[i * 4 + fld] = (T)stage[i];
+}
+template <typename T>
+__global__ void k_unpack_field(const T* __restrict__ q, double* __restrict__ stage, int fld, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) stage[i] = (double)q[i * 4 + fld];
+}
+
 // physical auxiliary fields for dg_get_fields: p_i00 = p*_i00 + S (29), p_ij0 by (32)
 template <typename T>
 __global__ void k_export_aux(Dev<T> d, int cur, double* face_aux, double* edge_aux) {
