@@ -38,7 +38,7 @@ typedef struct dg_solver dg_solver; /* opaque, owned by the library; free with d
 
 /* Tetrahedral mesh of a cuboid.  Any vertex order inside a tetrahedron is accepted
  * (negatively oriented cells are re-oriented internally).  The six planes bounding the vertex cloud are the
- * domain faces; all of them carry the HABC. */
+ * domain faces; each carries the HABC unless dg_options.face_bc says otherwise. */
 typedef struct {
     int32_t nverts;
     const double* xyz;   /* [nverts][3] */
@@ -61,6 +61,10 @@ typedef struct {
                                  (the choice at N = 5); 4 = experimental variant of 3 with the update in helper
                                  warps; 6 = experimental variant of 3 with a software-pipelined MMA loop;
                                  5 = fp32 tensor-core kernel (3xTF32, fp32-accurate), N = 3..5 (the choice there).  A kernel that does not cover (N, precision) gives DG_EINVAL */
+    int32_t face_bc[6];       /* boundary condition of the six domain faces, index axis * 2 + (1 for the face at the upper
+                                 end of the axis): 0 = HABC (the default), 1 = p = 0 (free surface),
+                                 2 = rigid wall (n.u = 0).  Auxiliary fields exist only on HABC faces, on the edges
+                                 between two of them and at the corners where three meet */
 } dg_options;
 
 typedef struct {
@@ -115,8 +119,9 @@ int dg_get_edge_map(const dg_solver* s, int32_t* axis, int32_t* normal_axes, int
  * Returns Np through *np_out. */
 int dg_reference_element(int dim, int N, double* rst, double* D, double* LIFT, int32_t* Fmask, int32_t* np_out);
 
-/* Host-side hierarchy sizes without touching the device: counts[0..3] = K, T, E, C. */
-int dg_mesh_counts(const dg_mesh* mesh, int32_t* counts);
+/* Host-side hierarchy sizes without touching the device: counts[0..3] = K, T, E, C.  face_bc: NULL (HABC on all
+ * faces) or the six codes of dg_options.face_bc. */
+int dg_mesh_counts(const dg_mesh* mesh, const int32_t* face_bc, int32_t* counts);
 
 /* Seconds of device time spent in each kernel family during the last dg_profile_step call (one time step run
  * with CUDA events around every launch; for per-kernel reporting, never inside a timed benchmark region).

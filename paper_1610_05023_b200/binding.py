@@ -24,7 +24,7 @@ class _Mesh(C.Structure):
 class _Options(C.Structure):
     _fields_ = [("precision", C.c_int32), ("cfl", C.c_double), ("dt", C.c_double), ("stream", C.c_void_p),
                 ("device", C.c_int32), ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64),
-                ("use_graph", C.c_int32), ("kernel", C.c_int32)]
+                ("use_graph", C.c_int32), ("kernel", C.c_int32), ("face_bc", C.c_int32 * 6)]
 
 
 class _Info(C.Structure):
@@ -85,10 +85,20 @@ def dg_reference_element(dim: int, N: int):
     return rst, D, LIFT, Fm
 
 
-def dg_mesh_counts(verts, tets):
+_BC_CODES = {"habc": 0, "dirichlet": 1, "rigid": 2}
+
+
+def _face_bc_codes(face_bc):
+    codes = np.zeros(6, dtype=np.int32)
+    for (axis, sign), kind in (face_bc or {}).items():
+        codes[axis * 2 + (1 if sign > 0 else 0)] = _BC_CODES[kind]
+    return codes
+
+
+def dg_mesh_counts(verts, tets, face_bc=None):
     m, keep = _mesh(verts, tets)
     out = np.zeros(4, dtype=np.int32)
-    _check(lib().dg_mesh_counts(C.byref(m), _ip(out)))
+    _check(lib().dg_mesh_counts(C.byref(m), _ip(_face_bc_codes(face_bc)), _ip(out)))
     return tuple(int(x) for x in out)
 
 
@@ -97,7 +107,9 @@ class Solver:
 
     def __init__(self, verts, tets, N: int, J: int, c, rho, precision: int = 64, cfl: float = 1.0,
                  dt: float = 0.0, device: int = 0, use_graph: bool = True, torch_workspace: bool = True,
-                 kernel: int = 0):
+                 kernel: int = 0, face_bc=None):
+        """face_bc: None (HABC everywhere) or {(axis, sign): "habc" | "dirichlet" | "rigid"} for some of the six domain
+        faces (axis 0..2, sign -1/+1) -- dg_options.face_bc."""
         import torch                                          # device memory + stream only
         if not torch.cuda.is_available():
             raise DgError("no CUDA device: the DG+HABC path has no CPU fallback")
@@ -108,6 +120,8 @@ class Solver:
         opt = _Options()
         opt.precision, opt.cfl, opt.dt, opt.device, opt.use_graph = precision, cfl, dt, device, int(use_graph)
         opt.kernel = int(kernel)
+        for i, code in enumerate(_face_bc_codes(face_bc)):
+            opt.face_bc[i] = int(code)
         self._torch = torch
         torch.cuda.set_device(device)
         # a dedicated (capturable) torch stream: the solver's kernels and CUDA graph run on it

@@ -158,6 +158,11 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
                 g[9 + f] = Zp / ((Zp + Zm) * Fs);
                 g[13 + f] = 1.0 / (Zp + Zm);
                 g[17 + f] = Fs;
+                // wall faces: the "neighbour" is the all-zero ghost row, so (u+ - u-, p+ - p-) = -(u-, p-); doubling
+                // one flux weight and dropping the other gives the mirror states p+ = -p- (p = 0)
+                // resp. n.u+ = -n.u- (rigid wall) through the same branch-free flux code
+                if (m.bc3[(size_t)k * 4 + f] == 1) { g[9 + f] = 0.0; g[13 + f] *= 2.0; }
+                else if (m.bc3[(size_t)k * 4 + f] == 2) { g[9 + f] *= 2.0; g[13 + f] = 0.0; }
                 const uint32_t fp = (uint32_t)(m.nbrface3[(size_t)k * 4 + f] | (m.nbrperm3[(size_t)k * 4 + f] << 2));
                 finfo[k] |= fp << (8 * f);
                 conn[(size_t)k * 4 + f] = nb >= 0 ? ((uint32_t)nb << 5) | fp : CONN_BND | ((uint32_t)(-1 - nb) << 5);
@@ -207,8 +212,8 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     const size_t n2 = (size_t)Tn * J * 3 * Nfp;
     d.fa[0] = U.zeros(n2); d.fa[1] = U.zeros(n2); d.fres = U.zeros(n2);
     d.S2 = U.zeros((size_t)std::max(m.T, 1) * Nfp);
-    d.qb3 = U.zeros((size_t)std::max(m.T, 1) * Nfp);
-    d.ghost3 = U.zeros((size_t)std::max(m.T, 1) * Nfp * 4);
+    d.qb3 = U.zeros((size_t)(m.T + 1) * Nfp);               // row T stays zero: the ghost of wall faces
+    d.ghost3 = U.zeros((size_t)(m.T + 1) * Nfp * 4);
     std::vector<double> geo2, d2, l2;
     std::vector<int> fm2;
     if (!A.dry) {
@@ -226,6 +231,8 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
                 if (nb >= 0) { const int kn = m.tri_tet[nb]; Zp = s->rho[kn] * s->c[kn]; }
                 g[13 + e] = Zp / (Zp + Zm);
                 g[16 + e] = 1.0 / (Zp + Zm);
+                if (m.bc2[(size_t)t * 3 + e] == 1) { g[13 + e] = 0.0; g[16 + e] *= 2.0; }
+                else if (m.bc2[(size_t)t * 3 + e] == 2) { g[13 + e] *= 2.0; g[16 + e] = 0.0; }
             }
             g[19] = s->rho[k] * s->c[k] * s->c[k]; g[20] = 1.0 / s->rho[k]; g[21] = s->c[k]; g[22] = Zm;
         }
@@ -247,7 +254,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     const size_t n1 = (size_t)E * J * J * 2 * N1;
     d.ea[0] = U.zeros(n1); d.ea[1] = U.zeros(n1); d.eres = U.zeros(n1);
     d.S1 = U.zeros((size_t)std::max(m.E, 1) * 2 * std::max(J, 1) * N1);
-    d.qb2 = U.zeros((size_t)std::max(m.E, 1) * 2 * std::max(J, 1) * N1);
+    d.qb2 = U.zeros((size_t)(2 * m.E + 1) * std::max(J, 1) * N1);    // row 2E stays zero
     std::vector<double> geo1;
     std::vector<int> slot, osign;
     if (!A.dry) {
@@ -263,6 +270,8 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
                 if (nb >= 0) { const int kn = m.tri_tet[m.lin_tri[nb * 2]]; Zp = s->rho[kn] * s->c[kn]; }
                 g[1 + e] = Zp / (Zp + Zm);
                 g[3 + e] = 1.0 / (Zp + Zm);
+                if (m.bc1[(size_t)l * 2 + e] == 1) { g[1 + e] = 0.0; g[3 + e] *= 2.0; }
+                else if (m.bc1[(size_t)l * 2 + e] == 2) { g[1 + e] *= 2.0; g[3 + e] = 0.0; }
             }
             g[5] = s->rho[k] * s->c[k] * s->c[k]; g[6] = 1.0 / s->rho[k]; g[7] = s->c[k];
             for (int side = 0; side < 2; ++side) {
@@ -280,7 +289,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.lin_osign = U.template ints<int>(osign, (size_t)m.E * 2);
     d.D1 = U.real(m.r1.D[0], (size_t)N1 * N1); d.L1 = U.real(m.r1.LIFT, (size_t)N1 * 2);
     // ---- 0D + algebra
-    d.qb1 = U.zeros((size_t)std::max(m.C, 1) * 3 * std::max(J * J, 1));
+    d.qb1 = U.zeros((size_t)(3 * m.C + 1) * std::max(J * J, 1));    // row 3C stays zero
     d.cor_line = U.template ints<int>(m.cor_line, (size_t)m.C * 3);
     d.cor_end = U.template ints<int>(m.cor_end, (size_t)m.C * 3);
     d.cor_sign = U.template ints<int>(m.cor_sign, (size_t)m.C * 3);
@@ -674,11 +683,11 @@ extern "C" {
 
 const char* dg_last_error(void) { return g_err.c_str(); }
 
-int dg_mesh_counts(const dg_mesh* mesh, int32_t* counts) {
+int dg_mesh_counts(const dg_mesh* mesh, const int32_t* face_bc, int32_t* counts) {
     try {
         if (!mesh || !counts) throw std::runtime_error("EINVAL: NULL argument");
         dg::HostMesh m;
-        dg::build_mesh(m, 1, mesh->nverts, mesh->xyz, mesh->ntets, mesh->tets);
+        dg::build_mesh(m, 1, mesh->nverts, mesh->xyz, mesh->ntets, mesh->tets, face_bc);
         counts[0] = m.K; counts[1] = m.T; counts[2] = m.E; counts[3] = m.C;
         return DG_OK;
     } catch (const std::exception& e) { return err_from_exception(e); }
@@ -775,7 +784,7 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured
         s->rho.assign(rho, rho + mesh->ntets);
         s->c.assign(c, c + mesh->ntets);
-        dg::build_mesh(s->m, N, mesh->nverts, mesh->xyz, mesh->ntets, mesh->tets);
+        dg::build_mesh(s->m, N, mesh->nverts, mesh->xyz, mesh->ntets, mesh->tets, opt ? opt->face_bc : nullptr);
         s->hc = dg::make_habc(J);
         // eq (46), PAPER.md:L796 (reading R7): dt = cfl * min_k 1 / (c_k (N+1)^2 max_f Fscale_kf)
         double dtmin = 1e300;

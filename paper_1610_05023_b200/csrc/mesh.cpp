@@ -40,7 +40,11 @@ int match_bary(const std::vector<ld>& bary, int nv, const int* cand, int ncand, 
 
 }  // namespace
 
-void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, const int32_t* tets) {
+void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, const int32_t* tets, const int* face_bc) {
+    for (int q = 0; q < 6; ++q) {
+        m.face_bc[q] = face_bc ? face_bc[q] : 0;
+        if (m.face_bc[q] < 0 || m.face_bc[q] > 2) throw std::runtime_error("EINVAL: face_bc codes are 0 (HABC), 1 (p = 0), 2 (rigid)");
+    }
     if (nverts < 4 || ntets < 1 || !xyz || !tets) fail("EINVAL: empty mesh");
     m.N = N; m.K = ntets;
     m.r3 = make_refelem(3, N); m.r2 = make_refelem(2, N); m.r1 = make_refelem(1, N);
@@ -162,6 +166,22 @@ void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, co
 
     // ---------------------------------------------------------------- surface mesh
     std::sort(bfaces.begin(), bfaces.end());
+    m.bc3.assign((size_t)K * 4, 0);
+    {
+        std::vector<int32_t> habc_faces, wall_faces;
+        for (int32_t bf : bfaces) {
+            int k = bf / 4, f = bf % 4;
+            int32_t v3[3];
+            for (int i = 0; i < 3; ++i) v3[i] = m.tets[(size_t)k * 4 + TET_FACE_VERTS[f][i]];
+            int pl[6][2];
+            if (planes_of(v3, 3, pl) != 1) fail("EINVAL: a boundary cell face does not lie on exactly one face of the bounding cuboid");
+            const int code = m.face_bc[pl[0][0] * 2 + (pl[0][1] > 0)];
+            if (code == 0) habc_faces.push_back(bf);
+            else { m.bc3[bf] = (uint8_t)code; wall_faces.push_back(bf); }
+        }
+        for (int32_t bf : wall_faces) m.nbr3[bf] = -1 - (int32_t)habc_faces.size();     // the zero ghost row
+        bfaces.swap(habc_faces);
+    }
     const int T = (int)bfaces.size();
     m.T = T;
     m.tri_tet.resize(T); m.tri_face.resize(T); m.tri_axis.resize(T); m.tri_sign.resize(T); m.tri_ax.resize((size_t)T * 2);
@@ -236,6 +256,7 @@ void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, co
 
     // ---------------------------------------------------------------- line mesh
     std::sort(bedges.begin(), bedges.end());
+    m.bc2.assign((size_t)T * 3, 0);
     std::map<std::pair<int32_t, int32_t>, int> line_of;
     std::vector<std::array<int32_t, 2>> lin_te;
     for (size_t q = 0; q < bedges.size(); ++q) {
@@ -247,6 +268,10 @@ void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, co
         for (int c = 0; c < np; ++c)
             if (pl[c][0] != m.tri_axis[t]) { if (oth >= 0) oth = -2; else oth = c; }
         if (np != 2 || oth < 0) fail("EINVAL: a boundary triangle edge without neighbour is not on an edge of the cuboid");
+        if (m.face_bc[pl[oth][0] * 2 + (pl[oth][1] > 0)] != 0) {       // the other face carries no HABC: wall condition, no line
+            m.bc2[bedges[q]] = (uint8_t)m.face_bc[pl[oth][0] * 2 + (pl[oth][1] > 0)];
+            continue;
+        }
         int a_own = m.tri_axis[t], a_oth = pl[oth][0];
         int side = a_own < a_oth ? 0 : 1;
         auto key = std::make_pair(std::min(vs[0], vs[1]), std::max(vs[0], vs[1]));
@@ -277,6 +302,8 @@ void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, co
     }
     const int E = (int)lin_te.size();
     m.E = E;
+    for (size_t q = 0; q < m.bc2.size(); ++q)
+        if (m.bc2[q]) m.nbr2[q] = -1 - 2 * E;                           // the zero ghost row
     m.lin_trinode.assign((size_t)E * 2 * N1, 0);
     for (int ell = 0; ell < E; ++ell)
         for (int side = 0; side < 2; ++side) {
@@ -291,6 +318,7 @@ void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, co
         }
     // line connectivity along each domain edge; unmatched ends are corners
     m.nbr1.assign((size_t)E * 2, INT32_MIN);
+    m.bc1.assign((size_t)E * 2, 0);
     std::vector<FaceKey> pk((size_t)E * 2);
     for (int ell = 0; ell < E; ++ell)
         for (int e = 0; e < 2; ++e) {
@@ -315,6 +343,11 @@ void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, co
             if (std::fabs(X(v, tang) - m.lo[tang]) < tol) s = -1;
             else if (std::fabs(X(v, tang) - m.hi[tang]) < tol) s = 1;
             else fail("EINVAL: a boundary line ends away from a corner of the cuboid");
+            if (m.face_bc[tang * 2 + (s > 0)] != 0) {                   // the third face carries no HABC: wall condition, no corner
+                m.bc1[pk[i].id] = (uint8_t)m.face_bc[tang * 2 + (s > 0)];
+                i = j;
+                continue;
+            }
             auto it = corner_of.find(v);
             int c;
             if (it == corner_of.end()) {
@@ -331,6 +364,8 @@ void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, co
         i = j;
     }
     m.C = (int)m.cor_vertex.size();
+    for (size_t q = 0; q < m.bc1.size(); ++q)
+        if (m.bc1[q]) m.nbr1[q] = -1 - 3 * m.C;                         // the zero ghost row
     for (size_t q = 0; q < m.cor_line.size(); ++q)
         if (m.cor_line[q] < 0) fail("EMESH: a corner is not the end of three boundary lines (F_bnd^lin = 3 K^pnt violated)");
 }

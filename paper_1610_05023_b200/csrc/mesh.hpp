@@ -21,12 +21,14 @@ struct HostMesh {
     std::vector<double> verts;           // [nv][3]
     std::vector<int32_t> tets;           // [K][4] positively oriented
     double lo[3], hi[3];                 // bounding box = the cuboid
+    int face_bc[6] = {0, 0, 0, 0, 0, 0}; // per domain face (axis * 2 + (outward sign > 0)): 0 HABC, 1 p = 0, 2 rigid wall
 
     // ---- volume level
     std::vector<double> G3;              // [K][9]  rx ry rz sx sy sz tx ty tz
     std::vector<double> J3;              // [K]     |det|
     std::vector<double> Fs3;             // [K][4]  sJ/J per face
-    std::vector<int32_t> nbr3;           // [K][4]  neighbour tet, or -1-t for the boundary triangle t
+    std::vector<int32_t> nbr3;           // [K][4]  neighbour tet, or -1-t for the boundary triangle t (t = T: wall face)
+    std::vector<uint8_t> bc3;            // [K][4]  0, or the wall type (1 p = 0, 2 rigid) of a boundary face without HABC
     std::vector<uint8_t> nbrface3;       // [K][4]  neighbour's local face
     std::vector<uint8_t> nbrperm3;       // [K][4]  index into perm3: neighbour face node = perm3[p][my face node]
     std::vector<uint8_t> perm3;          // [6][Nfp]
@@ -38,7 +40,8 @@ struct HostMesh {
     std::vector<double> J2;              // [T]
     std::vector<double> n2;              // [T][3][2] outward unit normals of the three edges (in-plane components)
     std::vector<double> Fs2;             // [T][3]
-    std::vector<int32_t> nbr2;           // [T][3]  neighbour triangle, or -1-(2*line+side) on a domain edge
+    std::vector<int32_t> nbr2;           // [T][3]  neighbour triangle, or -1-(2*line+side) on a domain edge (line = E: wall)
+    std::vector<uint8_t> bc2;            // [T][3]  wall type of a triangle edge that meets a domain face without HABC
     std::vector<int32_t> nbrnode2;       // [T][3][N1] neighbour's node (0..Nfp-1), or the line node (0..N) on a domain edge
 
     // ---- line level
@@ -49,7 +52,8 @@ struct HostMesh {
     std::vector<int32_t> lin_tri;        // [E][2] parent triangles on A, B
     std::vector<int32_t> lin_trinode;    // [E][2][N1] node of the parent triangle under each line node
     std::vector<double> J1;              // [E] length/2
-    std::vector<int32_t> nbr1;           // [E][2] neighbour line, or -1-(3*corner+axis) at a corner
+    std::vector<int32_t> nbr1;           // [E][2] neighbour line, or -1-(3*corner+axis) at a corner (corner = C: wall)
+    std::vector<uint8_t> bc1;            // [E][2] wall type of a line end that meets a domain face without HABC
 
     // ---- corners
     std::vector<int32_t> cor_vertex;     // [C]
@@ -60,6 +64,10 @@ struct HostMesh {
 
 // Throws std::runtime_error with a message starting "EMESH:" (degenerate / non-conforming mesh) or "EINVAL:"
 // (non-cuboid boundary).
-void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, const int32_t* tets);
+// face_bc: NULL (HABC on all six faces) or 6 codes indexed axis * 2 + (outward sign > 0): 0 HABC, 1 p = 0
+// (PAPER.md:L516-518), 2 rigid wall.  Only faces with code 0 get triangles; lines exist between two HABC faces and
+// corners where three meet (the K^pnt = 4 case of the paper's runs).
+void build_mesh(HostMesh& m, int N, int nverts, const double* xyz, int ntets, const int32_t* tets,
+                const int* face_bc = nullptr);
 
 }  // namespace dg

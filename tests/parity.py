@@ -33,9 +33,9 @@ def initial_on(w, x, y, z, c_elem, rho_elem):
     return w.fields(x, y, z, cn, rn)
 
 
-def run_oracle(w, nsteps=None, dt=None):
+def run_oracle(w, nsteps=None, dt=None, face_bc=None):
     from oracle.solver import OracleSolver
-    o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho, dt=dt)
+    o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho, dt=dt, face_bc=face_bc)
     x = o.nodes()
     o.set_initial(np.stack(initial_on(w, x[..., 0], x[..., 1], x[..., 2], w.c, w.rho)))
     o.step(w.nsteps if nsteps is None else nsteps)
@@ -44,9 +44,10 @@ def run_oracle(w, nsteps=None, dt=None):
                 xe=o.H.lin.x if o.E else np.zeros((0, 1, 3)), T=o.T, E=o.E, C=o.C)
 
 
-def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True, kernel=0):
+def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True, kernel=0, face_bc=None):
     from paper_1610_05023_b200 import Solver
-    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=precision, dt=dt, use_graph=use_graph, kernel=kernel)
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=precision, dt=dt, use_graph=use_graph, kernel=kernel,
+               face_bc=face_bc)
     x, y, z = s.get_nodes()
     s.set_initial(*initial_on(w, x, y, z, w.c, w.rho))
     s.step(w.nsteps if nsteps is None else nsteps)

@@ -95,6 +95,35 @@ def test_3d_kernel_variants_fp32(N, kernel):
         assert err["p"] <= 4 * ref["p"] + 1e-7 and err["u"] <= 4 * ref["u"] + 1e-7, (err, ref)
 
 
+FREE_SURFACE = {(2, -1): "dirichlet"}
+BC_CASES = {
+    "free_surface": FREE_SURFACE,                                          # 5 HABC faces, 8 edges, 4 corners
+    "habc_x_rigid_yz": {(1, -1): "rigid", (1, 1): "rigid", (2, -1): "rigid", (2, 1): "rigid"},   # faces only, no edges
+    "mixed": {(0, -1): "dirichlet", (0, 1): "rigid", (1, 1): "dirichlet"},  # HABC on -y, -z, +z: 2 edges, no corner
+    "all_walls": {(a, sg): ("dirichlet" if a else "rigid") for a in range(3) for sg in (-1, 1)},
+}
+
+
+@pytest.mark.parametrize("case", sorted(BC_CASES))
+@pytest.mark.parametrize("N,prec,kernel", [(3, 64, 0), (5, 64, 0), (4, 64, 1), (5, 32, 0), (6, 32, 0)])
+def test_mixed_boundary_conditions(case, N, prec, kernel):
+    """dg_options.face_bc: p = 0 and rigid walls on some domain faces, HABC on the others, auxiliary
+    fields only where HABC faces meet -- against the oracle's per-face boundary flags, through every 3D kernel."""
+    face_bc = BC_CASES[case]
+    w = make_workload("cfg1", n=3, N=N, J=3, nsteps=60)
+    lib = parity.run_library(w, precision=prec, kernel=kernel, face_bc=face_bc)
+    ora = parity.run_oracle(w, face_bc=face_bc)
+    assert (lib["T"], lib["E"], lib["C"]) == (ora["T"], ora["E"], ora["C"])
+    err = parity.compare(lib, ora)
+    for k in ("p", "u", "face", "edge"):
+        if k in err:
+            assert err[k] <= TOL[prec], (k, err)
+    assert ("face" in err) == (ora["T"] > 0) and ("edge" in err) == (ora["E"] > 0)
+    if case == "free_surface":
+        assert (lib["T"], lib["E"], lib["C"]) == (5 * 18, 8 * 3, 4)
+        assert err["norm_face"] > 1e-3 * err["norm_p"] and err["norm_edge"] > 1e-5 * err["norm_p"], err
+
+
 def test_edge_cases():
     """Smallest mesh (one hex, 6 tets: every tet touches the boundary), J=1, J=12 (maximum), graph off,
     negatively oriented input cells, zero initial data, nsteps=0."""

@@ -49,6 +49,29 @@ def test_mesh_counts_match_oracle(n):
     assert pkg.dg_mesh_counts(v, t2)[0] == K
 
 
+@pytest.mark.parametrize("face_bc", [
+    {(2, -1): "dirichlet"},                                              # free surface: 5 HABC faces, 8 edges, 4 corners
+    {(1, -1): "rigid", (1, 1): "rigid", (2, -1): "rigid", (2, 1): "rigid"},  # HABC on the two x faces only
+    {(0, -1): "dirichlet", (0, 1): "rigid", (1, 1): "dirichlet"},
+    {(a, s): "dirichlet" for a in range(3) for s in (-1, 1)},             # no auxiliary level at all
+])
+def test_mixed_boundary_hierarchy_matches_oracle(face_bc):
+    """dg_options.face_bc: triangles only on HABC faces, lines between two of
+    them, corners where three meet -- the same counts as the oracle's hierarchy builder."""
+    n = 3
+    v, t = cube_mesh(n)
+    K = len(t)
+    H = build_hierarchy(v, t, 1, np.ones(K), np.ones(K), face_bc)
+    nh = 6 - len(face_bc)
+    got = pkg.dg_mesh_counts(v, t, face_bc)
+    size = lambda level: 0 if level is None else level.K
+    ncor = 0 if getattr(H, "cor_vertex", None) is None else H.cor_vertex.size
+    assert got == (K, size(H.tri), size(H.lin), ncor)
+    assert got[1] == 2 * n * n * nh
+    if face_bc == {(2, -1): "dirichlet"}:
+        assert got[2:] == (8 * n, 4)                                      # the paper's K^pnt = 4 configuration
+
+
 def test_error_codes():
     lib = pkg.lib()
     v, t = cube_mesh(2)
@@ -65,3 +88,6 @@ def test_error_codes():
     assert lib.dg_workspace_bytes(ctypes.byref(m), 3, 2, 64, ctypes.byref(nbytes)) == 0 and nbytes.value > 48 * 20 * 4 * 8 * 3
     assert lib.dg_workspace_bytes(ctypes.byref(m), 3, 13, 64, ctypes.byref(nbytes)) == -1
     assert lib.dg_workspace_bytes(ctypes.byref(m), 3, 2, 16, ctypes.byref(nbytes)) == -1
+    bad = np.array([0, 0, 3, 0, 0, 0], dtype=np.int32)
+    out = np.zeros(4, dtype=np.int32)
+    assert lib.dg_mesh_counts(ctypes.byref(m), pkg.binding._ip(bad), pkg.binding._ip(out)) == -1
