@@ -92,7 +92,7 @@ def oracle_sample(workload: str, precision: int, budget_s: float = 20.0):
     d = CONFIGS[workload]
     n = min(d["n"], 8)
     w = make_workload(workload, n=n)
-    o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho)
+    o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho, face_bc=w.face_bc)
     x = o.nodes()
     cn = np.repeat(w.c[:, None], x.shape[1], axis=1)
     o.set_initial(np.stack(w.fields(x[..., 0], x[..., 1], x[..., 2], cn, 1.0)))
@@ -106,7 +106,7 @@ def oracle_sample(workload: str, precision: int, budget_s: float = 20.0):
             break
     nodes = o.H.tet.K * o.H.tet.ref.Np
     cores = len(os.sched_getaffinity(0))
-    desc = f"{workload} rule on a {n}^3 hex grid ({o.H.tet.K} tets, N={w.N}, J={w.J}), {steps} steps, fp64 numpy"
+    desc = f"{workload} rule on a {'x'.join(str(m) for m in w.shape)} hex grid ({o.H.tet.K} tets, N={w.N}, J={w.J}), {steps} steps, fp64 numpy"
     return nodes * steps / el, desc, cores, el / steps
 
 
@@ -163,7 +163,7 @@ def main():
     w = make_workload(args.workload, n=args.n, N=args.N, J=args.J)
     prec = args.precision
     t_setup = time.perf_counter()
-    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, kernel=args.kernel)
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, kernel=args.kernel, face_bc=w.face_bc)
     x, y, z = s.get_nodes()
     cn = np.repeat(w.c[:, None], s.Np, axis=1)
     fields = [np.ascontiguousarray(f) for f in w.fields(x, y, z, cn, 1.0)]
@@ -255,7 +255,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": f"f{prec}", "data": "synthetic",
-            "config": {"workload": args.workload, "n_hex": w.n, "N": w.N, "J": w.J, "K": info["K"], "T": info["T"],
+            "config": {"workload": args.workload, "n_hex": w.n, "hex_grid": list(w.shape), "N": w.N, "J": w.J, "K": info["K"], "T": info["T"],
                        "E": info["E"], "corners": info["C"], "nodes": nodes, "dt": info["dt"],
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "state (q,res) exceeds L2 many times over; no flush needed",

@@ -35,6 +35,7 @@ def initial_on(w, x, y, z, c_elem, rho_elem):
 
 def run_oracle(w, nsteps=None, dt=None, face_bc=None):
     from oracle.solver import OracleSolver
+    face_bc = getattr(w, "face_bc", None) if face_bc is None else face_bc
     o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho, dt=dt, face_bc=face_bc)
     x = o.nodes()
     o.set_initial(np.stack(initial_on(w, x[..., 0], x[..., 1], x[..., 2], w.c, w.rho)))
@@ -46,6 +47,7 @@ def run_oracle(w, nsteps=None, dt=None, face_bc=None):
 
 def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True, kernel=0, face_bc=None):
     from paper_1610_05023_b200 import Solver
+    face_bc = getattr(w, "face_bc", None) if face_bc is None else face_bc
     s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=precision, dt=dt, use_graph=use_graph, kernel=kernel,
                face_bc=face_bc)
     x, y, z = s.get_nodes()

@@ -124,6 +124,17 @@ def test_mixed_boundary_conditions(case, N, prec, kernel):
         assert err["norm_face"] > 1e-3 * err["norm_p"] and err["norm_edge"] > 1e-5 * err["norm_p"], err
 
 
+@pytest.mark.parametrize("prec", [64, 32])
+def test_seam_shaped_workload(prec):
+    """the SEAM-shaped stand-in (cuboid 3.5 x 4 x 1.5, free surface on top, HABC on the other five faces,
+    strongly heterogeneous c AND rho varying from cell to cell, N = 3, J = 3) on a 7 x 8 x 3 hex grid."""
+    w = make_workload("seam", n=7, nsteps=80)
+    assert w.shape == (7, 8, 3) and w.face_bc == {(2, 1): "dirichlet"} and np.unique(w.rho).size > 100
+    lib, ora = parity.run_library(w, precision=prec), parity.run_oracle(w)
+    assert (lib["T"], lib["E"], lib["C"]) == (ora["T"], ora["E"], ora["C"]) == (2 * (7 * 8 + 2 * 7 * 3 + 2 * 8 * 3), 4 * 3 + 2 * 7 + 2 * 8, 4)
+    _check(parity.compare(lib, ora), prec)
+
+
 def test_edge_cases():
     """Smallest mesh (one hex, 6 tets: every tet touches the boundary), J=1, J=12 (maximum), graph off,
     negatively oriented input cells, zero initial data, nsteps=0."""

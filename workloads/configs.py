@@ -9,6 +9,10 @@ Recipe (also stated in DESIGN.md §4):
     (layer index from the hex z-index), speeds drawn from U[lo,hi] with the config's seed.
   * initial data: Gaussian pressure pulse exp(-|x-x0|^2 / (2 w^2)), w = 0.2, seeded centre; optionally a
     superposed plane wave p = A cos(2 pi k.x), u = k p / (rho c) with a seeded unit direction k.
+  * "seam": a cuboid with the aspect of the paper's SEAM Phase I run (35 x 40 x 15 km -> 3.5 x 4.0 x 1.5):
+    70 x 80 x 30 hexahedra = 1,008,000 tetrahedra (the paper's mesh: 1,179,989), N = 3, J = 3, free surface (p = 0) on
+    the top face and HABC on the other five, strongly heterogeneous c and rho (depth gradient 1.5 -> 3.5, a fast
+    4.5 inclusion, seeded +-3 % cell-to-cell variation; rho = 1 + (c - 1.5) / 4).  The SEAM model itself is not available.
   * seeds: 1610_05023 + config index, numpy PCG64.
 The paper's own meshes (70,895-tet cube, SEAM Phase I model) are not available; these stand in for them.
 """
@@ -40,6 +44,8 @@ class Workload:
     plane_dir: np.ndarray | None
     plane_amp: float
     seed: int
+    shape: tuple = None         # hexes per axis (n, n, n for the cube configs)
+    face_bc: dict = None        # {(axis, sign): "dirichlet" | "rigid"} for domain faces without HABC (None: HABC everywhere)
 
     @property
     def K(self) -> int:
@@ -50,21 +56,28 @@ class Workload:
 
 
 def cube_mesh(n: int, perturb: float = 0.0, rng: np.random.Generator | None = None):
-    """Kuhn 6-tet split of an n^3 hex grid on [-1,1]^3.  Element order: hex-major (x fastest), the six
-    tets of a hex consecutive.  Returns (verts[nv,3] f64, tets[K,4] i32), all tets positively oriented."""
-    g = np.linspace(-1.0, 1.0, n + 1)
-    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    """Kuhn 6-tet split of an n^3 hex grid on [-1,1]^3 (see box_mesh)."""
+    return box_mesh((n, n, n), ((-1.0, 1.0),) * 3, perturb, rng)
+
+
+def box_mesh(shape, box, perturb: float = 0.0, rng: np.random.Generator | None = None):
+    """Kuhn 6-tet split of an nx x ny x nz hex grid on the cuboid `box` = ((x0,x1),(y0,y1),(z0,z1)).  Element order:
+    hex-major (x fastest), the six tets of a hex consecutive.  Returns (verts[nv,3] f64, tets[K,4] i32), all tets
+    positively oriented."""
+    nx, ny, nz = shape
+    gx, gy, gz = (np.linspace(b[0], b[1], m + 1) for b, m in zip(box, shape))
+    X, Y, Z = np.meshgrid(gx, gy, gz, indexing="ij")
     verts = np.stack([X.ravel(), Y.ravel(), Z.ravel()], axis=1).astype(np.float64)
 
     def vid(i, j, k):
-        return (i * (n + 1) + j) * (n + 1) + k
+        return (i * (ny + 1) + j) * (nz + 1) + k
 
     if perturb > 0.0:
         assert rng is not None
-        h = 2.0 / n
-        I, Jx, Kx = np.meshgrid(np.arange(n + 1), np.arange(n + 1), np.arange(n + 1), indexing="ij")
-        interior = ((I > 0) & (I < n) & (Jx > 0) & (Jx < n) & (Kx > 0) & (Kx < n)).ravel()
-        d = rng.uniform(-perturb * h, perturb * h, size=verts.shape)
+        h = np.array([(b[1] - b[0]) / m for b, m in zip(box, shape)])
+        I, Jx, Kx = np.meshgrid(np.arange(nx + 1), np.arange(ny + 1), np.arange(nz + 1), indexing="ij")
+        interior = ((I > 0) & (I < nx) & (Jx > 0) & (Jx < ny) & (Kx > 0) & (Kx < nz)).ravel()
+        d = rng.uniform(-perturb, perturb, size=verts.shape) * h
         verts[interior] += d[interior]
 
     # the six monotone lattice paths (0,0,0)->(1,1,1): one tet per permutation of the axes
@@ -78,9 +91,9 @@ def cube_mesh(n: int, perturb: float = 0.0, rng: np.random.Generator | None = No
         corner_paths.append(np.array(path))            # [4,3]
     corner_paths = np.array(corner_paths)              # [6,4,3]
 
-    kk, jj, ii = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")  # x fastest
+    kk, jj, ii = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")  # x fastest
     hexes = np.stack([ii.ravel(), jj.ravel(), kk.ravel()], axis=1)                        # [n^3,3]
-    cidx = hexes[:, None, None, :] + corner_paths[None, :, :, :]                          # [n^3,6,4,3]
+    cidx = hexes[:, None, None, :] + corner_paths[None, :, :, :]                          # [hexes,6,4,3]
     tets = vid(cidx[..., 0], cidx[..., 1], cidx[..., 2]).reshape(-1, 4)
     # orient positively
     a = verts[tets[:, 1]] - verts[tets[:, 0]]
@@ -120,6 +133,30 @@ def initial_fields(w: Workload, x, y, z, c_node, rho_node):
     return p, u, v, ww
 
 
+SEAM_BOX = ((0.0, 3.5), (0.0, 4.0), (0.0, 1.5))
+
+
+def seam_shape(n: int):
+    """hexes per axis of the SEAM-shaped cuboid with n hexes along x (70 -> 70 x 80 x 30)"""
+    return (n, max(1, round(n * 8 / 7)), max(1, round(n * 3 / 7)))
+
+
+def seam_materials(shape, box, rng: np.random.Generator):
+    """(c, rho) per tetrahedron of the SEAM-shaped stand-in: depth gradient + fast inclusion + seeded variation."""
+    nx, ny, nz = shape
+    cen = [b[0] + (np.arange(m) + 0.5) * (b[1] - b[0]) / m for b, m in zip(box, shape)]
+    Zc, Yc, Xc = np.meshgrid(cen[2], cen[1], cen[0], indexing="ij")           # hex-major, x fastest
+    L = [b[1] - b[0] for b in box]
+    depth = (box[2][1] - Zc) / L[2]
+    c = 1.5 + 2.0 * depth
+    inside = ((Xc - 0.55 * L[0]) / (0.2 * L[0])) ** 2 + ((Yc - 0.5 * L[1]) / (0.25 * L[1])) ** 2 \
+        + ((Zc - 0.45 * L[2]) / (0.25 * L[2])) ** 2 < 1.0
+    c = np.where(inside, 4.5, c)
+    c = c * (1.0 + 0.03 * rng.uniform(-1.0, 1.0, size=c.shape))
+    rho = 1.0 + (c - 1.5) / 4.0
+    return np.repeat(c.ravel(), 6).astype(np.float64), np.repeat(rho.ravel(), 6).astype(np.float64)
+
+
 # name -> static description (BASELINE.json configs[0..4]); config 4 is a sweep, see `sweep`.
 CONFIGS = {
     "cfg1": dict(index=1, n=2, N=3, J=2, nsteps=100, precisions=("f64",), c=("const", 1.0),
@@ -133,6 +170,9 @@ CONFIGS = {
                  sweep=dict(N=tuple(range(1, 9)), J=(0, 4, 8))),
     "cfg5": dict(index=5, n=64, N=5, J=8, nsteps=100, precisions=("f64", "f32"),
                  c=("layers", 4, 1.5, 4.5), pulse="corner", plane=False, perturb=0.0),
+    # SEAM-shaped workload (not one of BASELINE's five configs; see the module docstring)
+    "seam": dict(index=6, n=70, N=3, J=3, nsteps=100, precisions=("f32", "f64"), c=("seam",), pulse="seam",
+                 plane=False, perturb=0.0, face_bc={(2, 1): "dirichlet"}),
 }
 
 
@@ -146,17 +186,26 @@ def make_workload(name: str, *, n: int | None = None, N: int | None = None, J: i
     J = d["J"] if J is None else J
     nsteps = d["nsteps"] if nsteps is None else nsteps
     rng = np.random.default_rng(SEED0 + d["index"])
-    verts, tets = cube_mesh(n, d["perturb"], rng)
+    if name == "seam":
+        shape, box = seam_shape(n), SEAM_BOX
+    else:
+        shape, box = (n, n, n), ((-1.0, 1.0),) * 3
+    verts, tets = box_mesh(shape, box, d["perturb"], rng)
     K = tets.shape[0]
+    rho = np.ones(K, dtype=np.float64)
     if d["c"][0] == "const":
         c = np.full(K, d["c"][1], dtype=np.float64)
+    elif d["c"][0] == "seam":
+        c, rho = seam_materials(shape, box, rng)
     else:
         _, nl, lo, hi = d["c"]
         c = layered_speed(n, nl, lo, hi, rng)
-    rho = np.ones(K, dtype=np.float64)
     jitter = rng.uniform(-1.0, 1.0, size=3)
     if d["pulse"] == "centre":
         centre = 0.3 * jitter / max(1.0, np.linalg.norm(jitter))        # |x0| < 0.3
+    elif d["pulse"] == "seam":
+        # near the bottom (+x, +y, -z) corner: three HABC faces, their edges and a corner carry data from t = 0
+        centre = np.array([box[0][1] - 0.3, box[1][1] - 0.3, box[2][0] + 0.3]) + 0.03 * jitter
     else:
         # near the (+,+,+) corner so that faces, edges and one corner carry O(0.1) data at t=0
         # (the stated step counts cover too little time for a central pulse to arrive)
@@ -167,7 +216,7 @@ def make_workload(name: str, *, n: int | None = None, N: int | None = None, J: i
         plane_dir = k / np.linalg.norm(k)
     return Workload(name=name, n=n, N=N, J=J, nsteps=nsteps, precisions=d["precisions"], verts=verts,
                     tets=tets, c=c, rho=rho, pulse_centre=centre, pulse_width=0.2, plane_dir=plane_dir,
-                    plane_amp=0.5, seed=SEED0 + d["index"])
+                    plane_amp=0.5, seed=SEED0 + d["index"], shape=shape, face_bc=d.get("face_bc"))
 
 
 def scaled_workload(name: str, n: int, nsteps: int) -> Workload:
