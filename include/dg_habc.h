@@ -97,6 +97,13 @@ int dg_get_nodes(const dg_solver* s, double* x, double* y, double* z);
  * incoming characteristics are initialised by running the closure chain once on the device. */
 int dg_set_initial(dg_solver* s, const double* p, const double* u, const double* v, const double* w);
 
+/* Point source delta(x - xyz) * amplitude * S(t) in the pressure equation, S(t) = (t - t_s)
+ * exp(-pi^2 f_peak^2 (t - t_s)^2) being the time integral of the Ricker wavelet, eq (44).  The delta is projected
+ * onto the cell that contains xyz (the first one, in the caller's order, whose barycentric coordinates are all
+ * >= -1e-12).  Time starts at 0 at dg_set_initial; stage n of a step evaluates S at t + c_n dt (LSRK, L531-540).
+ * amplitude = 0 switches the source off.  xyz: [3], host. */
+int dg_set_source(dg_solver* s, const double* xyz, double f_peak, double t_s, double amplitude);
+
 /* Advance nsteps time steps of 5 LSRK stages each (eq (42)-(43), L531-540; kernel order L627). Asynchronous. */
 int dg_step(dg_solver* s, int nsteps);
 

@@ -120,6 +120,8 @@ class OracleSolver:
             self.Lc, self.Tc = habc.corner_system(J)
         # eq (46), reading R7: dt = cfl * min_k 1 / (c_k (N+1)^2 Fscale_k), Fscale_k = max_f sJ_f/J_k
         self.dt = float(dt) if dt else cfl * float(np.min(1.0 / (H.tet.c * (N + 1) ** 2 * H.tet.Fs.max(axis=1))))
+        self._verts, self._tets = np.asarray(verts, dtype=np.float64), np.asarray(tets)
+        self.source = None
         self.set_initial(np.zeros((4, H.tet.K, H.tet.ref.Np)))
 
     # ------------------------------------------------------------------ state
@@ -133,6 +135,34 @@ class OracleSolver:
         self.fa = np.zeros((J, 3, self.T, H.tet.ref.Nfp))
         self.ea = np.zeros((J, J, 2, self.E, self.N + 1))
         self.res = None
+        self.t = 0.0
+
+    # ------------------------------------------------------------------ point source (eq (44))
+    def set_source(self, xs, f_peak: float, t_s: float, amplitude: float = 1.0):
+        """Dirac source delta(x - xs) * amplitude * S(t) in the pressure equation (L780), S(t) = (t - t_s)
+        exp(-pi^2 f_peak^2 (t - t_s)^2) the integral of the Ricker wavelet (44) (L784).  Galerkin projection onto
+        the cell that contains xs (the first one in the caller's order whose barycentric coordinates are all
+        >= -1e-12):  M J dp/dt = ... + l(xs) S  =>  dp_n/dt += S (M^-1 l(r_s))_n / J,  M^-1 l(r) = V psi(r)."""
+        xs = np.asarray(xs, dtype=np.float64)
+        V4 = self._verts[self._tets]                                     # [K,4,3]
+        A = np.transpose(V4[:, 1:] - V4[:, :1], (0, 2, 1))               # columns = edge vectors
+        lam = np.linalg.solve(A, np.broadcast_to(xs - V4[:, 0], (len(V4), 3))[..., None])[..., 0]
+        bary = np.concatenate([1.0 - lam.sum(axis=1, keepdims=True), lam], axis=1)
+        inside = np.nonzero(bary.min(axis=1) >= -1e-12)[0]
+        if inside.size == 0:
+            raise ValueError("the source point is outside the mesh")
+        k = int(inside[0])
+        r, s_, t_ = (-1.0 + 2.0 * bary[k, 1 + a] for a in range(3))
+        from .refelem import vandermonde
+        LD = np.longdouble
+        psi, _ = vandermonde(3, self.N, np.array([r], dtype=LD), np.array([s_], dtype=LD), np.array([t_], dtype=LD))
+        w = (self.H.tet.ref.V @ np.asarray(psi[0], dtype=np.float64)) / self.H.tet.detJ[k]
+        self.source = dict(k=k, w=w, f=float(f_peak), ts=float(t_s), amp=float(amplitude))
+
+    def source_S(self, t):
+        src = self.source
+        tau = t - src["ts"]
+        return src["amp"] * tau * np.exp(-(np.pi * src["f"] * tau) ** 2)
 
     def state(self):
         return (self.q, self.fa, self.ea)
@@ -209,12 +239,15 @@ class OracleSolver:
         return out
 
     # ------------------------------------------------------------------ F(y)
-    def rhs(self, y):
+    def rhs(self, y, t=None):
+        """F(y) (autonomous), plus the point source evaluated at time t when one is set."""
         q, fa, ea = y
         H, J, cn = self.H, self.J, self.cn
         cl = self.closures(y)
         rp, rU = dg_rhs(H.tet, q[0][None], q[1:4][None], cl["rm_tet"])
         dq = np.concatenate([rp, rU[0]], axis=0)
+        if self.source is not None and t is not None:
+            dq[0, self.source["k"]] += self.source_S(t) * self.source["w"]
         dfa, dea = np.zeros_like(fa), np.zeros_like(ea)
         if self.T and J:
             rp, rU = dg_rhs(H.tri, cl["p_face"], fa[:, 1:3], cl["rm_tri"])
@@ -235,10 +268,11 @@ class OracleSolver:
         s = [np.zeros_like(a) for a in y]
         for _ in range(nsteps):
             for n in range(5):
-                F = self.rhs(tuple(y))
+                F = self.rhs(tuple(y), self.t + RK4C[n] * self.dt)
                 for a in range(3):
                     s[a] = RK4A[n] * s[a] + self.dt * F[a]
                     y[a] = y[a] + RK4B[n] * s[a]
+            self.t += self.dt
         self.q, self.fa, self.ea = y
 
     # ------------------------------------------------------------------ outputs (DESIGN.md §3 O8)

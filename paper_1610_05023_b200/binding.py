@@ -33,7 +33,7 @@ class _Info(C.Structure):
                 ("launches_per_step", C.c_int32), ("dt", C.c_double), ("device_bytes", C.c_uint64)]
 
 
-EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_step",
+EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_set_source", "dg_step",
            "dg_get_fields", "dg_get_face_map", "dg_get_edge_map", "dg_reference_element", "dg_mesh_counts",
            "dg_profile_step", "dg_last_error", "dg_destroy"]
 
@@ -151,6 +151,18 @@ class Solver:
     def set_initial(self, p, u, v, w):
         a = [np.ascontiguousarray(f, dtype=np.float64).reshape(self.K, self.Np) for f in (p, u, v, w)]
         _check(lib().dg_set_initial(self._h, *[_dp(f) for f in a]))
+
+    def set_source(self, xyz, f_peak: float, t_s: float, amplitude: float = 1.0):
+        xyz = np.ascontiguousarray(xyz, dtype=np.float64).reshape(3)
+        L = lib()
+        L.dg_set_source.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.c_double, C.c_double, C.c_double]
+        _check(L.dg_set_source(self._h, _dp(xyz), float(f_peak), float(t_s), float(amplitude)))
+        self.launches_per_step = self.info["launches_per_step"] = self._refresh_info()["launches_per_step"]
+
+    def _refresh_info(self):
+        info = _Info()
+        _check(lib().dg_get_info(self._h, C.byref(info)))
+        return {k: getattr(info, k) for k, _ in _Info._fields_}
 
     def step(self, nsteps: int = 1):
         _check(lib().dg_step(self._h, int(nsteps)))

@@ -43,6 +43,8 @@ void cu(cudaError_t e, const char* what) {
 // LSRK4(5) of Carpenter & Kennedy (ref. [10] of the paper; eq (42)-(43))
 const double RKA[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
                        -3550918686646.0 / 2091501179385.0, -1275806237668.0 / 842570457699.0};
+const double RKC[5] = {0.0, 1432997174477.0 / 9575080441755.0, 2526269341429.0 / 6820363962896.0,
+                       2006345519317.0 / 3224310063776.0, 2802321613138.0 / 2924317926251.0};
 const double RKB[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 13612068292357.0,
                        1720146321549.0 / 2090206949498.0, 3134564353537.0 / 4481467310338.0,
                        2277821191437.0 / 14882151754819.0};
@@ -87,6 +89,12 @@ struct dg_solver {
     bool use_graph = true;
     cudaGraphExec_t graph[2] = {nullptr, nullptr};
     std::vector<double> rho, c;
+    // point source (dg_set_source): cell, Ricker parameters, device copies of the weights and of the simulated time
+    bool src_on = false;
+    int src_k = 0;
+    double src_f = 0, src_ts = 0, src_amp = 0;
+    void* src_w = nullptr;          // [Np] of T
+    double* t_dev = nullptr;        // simulated time at the start of the current step
     double* export_buf = nullptr;   // device scratch for dg_get_fields (aux fields, fp64)
     size_t export_elems = 0;
 };
@@ -307,6 +315,12 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.PeT = U.real(transposed(h.Pe, 2 * J), e2);
     d.QeT = U.real(transposed(h.Qe, 2 * J), e2);
     d.Gc = U.real(h.Gc, c2);
+    s->src_w = A.take(sizeof(T) * Np);
+    s->t_dev = (double*)A.take(sizeof(double));
+    if (!A.dry) {
+        cu(cudaMemset(s->src_w, 0, sizeof(T) * Np), "memset");
+        cu(cudaMemset(s->t_dev, 0, sizeof(double)), "memset");
+    }
     // fp64 scratch for exporting the physical auxiliary fields
     s->export_elems = n2 + n1;
     s->export_buf = (double*)A.take(sizeof(double) * std::max<size_t>(s->export_elems, 1));
@@ -512,9 +526,17 @@ void launch_closures(dg_solver* s, Dev<T>& d, int cur) {
 }
 
 template <typename T>
+void launch_source(dg_solver* s, Dev<T>& d, int src, int stage) {
+    if (!s->src_on) return;
+    k_source<T><<<1, 64, 0, s->stream>>>(d.q[src ^ 1], d.res, (const T*)s->src_w, s->src_k, d.Np, s->t_dev,
+                                       RKC[stage] * s->dt, s->dt, RKB[stage], s->src_f, s->src_ts, s->src_amp, stage == 4);
+}
+
+template <typename T>
 void launch_stage(dg_solver* s, Dev<T>& d, int src, int stage) {
     const double a = RKA[stage], b = RKB[stage];
     launch_vol3d<T>(s, d, src, a, b, false);
+    launch_source<T>(s, d, src, stage);
     if (d.J > 0 && d.Tn > 0) {
         launch_face2d<T>(s, d, src, a, b);
         if (d.E > 0) {
@@ -527,7 +549,7 @@ void launch_stage(dg_solver* s, Dev<T>& d, int src, int stage) {
 }
 
 int launches_per_stage(const dg_solver* s) {
-    int n = 1;
+    int n = 1 + (s->src_on ? 1 : 0);
     if (s->J > 0 && s->m.T > 0) {
         n += 2;                       // 2D solver + face closure
         if (s->m.E > 0) n += 2;       // 1D solver + edge closure
@@ -604,6 +626,7 @@ void upload_initial(dg_solver* s, Dev<T>& d, const double* p, const double* u, c
     if (n2) cu(cudaMemsetAsync(d.fres, 0, sizeof(T) * n2, s->stream), "memset");
     if (n1) cu(cudaMemsetAsync(d.eres, 0, sizeof(T) * n1, s->stream), "memset");
     s->cur = 0;
+    cu(cudaMemsetAsync(s->t_dev, 0, sizeof(double), s->stream), "memset");
     launch_closures<T>(s, d, 0);        // reading R5: cached r^-, S consistent with the initial state
     cu(cudaStreamSynchronize(s->stream), "set_initial");
 }
@@ -650,7 +673,7 @@ void profile_step(dg_solver* s, Dev<T>& d, double* ms) {
     for (int st = 0; st < 5; ++st) {
         const int src = s->cur;
         const double a = RKA[st], b = RKB[st];
-        timed(0, [&] { launch_vol3d<T>(s, d, src, a, b, false); });
+        timed(0, [&] { launch_vol3d<T>(s, d, src, a, b, false); launch_source<T>(s, d, src, st); });
         if (d.J > 0 && d.Tn > 0) {
             timed(1, [&] { launch_face2d<T>(s, d, src, a, b); });
             if (d.E > 0) {
@@ -864,6 +887,61 @@ int dg_set_initial(dg_solver* s, const double* p, const double* u, const double*
         cu(cudaSetDevice(s->device), "cudaSetDevice");
         if (s->precision == 64) upload_initial<double>(s, s->d64, p, u, v, w);
         else upload_initial<float>(s, s->d32, p, u, v, w);
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
+
+int dg_set_source(dg_solver* s, const double* xyz, double f_peak, double t_s, double amplitude) {
+    try {
+        if (!s || !xyz) throw std::runtime_error("EINVAL: NULL argument");
+        if (!(f_peak > 0)) throw std::runtime_error("EINVAL: f_peak must be positive");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        const dg::HostMesh& m = s->m;
+        typedef long double ld;
+        int kfound = -1;
+        ld lam[4] = {0, 0, 0, 0};
+        for (int k = 0; k < m.K && kfound < 0; ++k) {
+            const double* v[4];
+            for (int i = 0; i < 4; ++i) v[i] = &m.verts[(size_t)m.tets[(size_t)k * 4 + i] * 3];
+            ld A[3][3], b[3];
+            for (int r = 0; r < 3; ++r) {
+                for (int c = 0; c < 3; ++c) A[r][c] = (ld)v[c + 1][r] - (ld)v[0][r];
+                b[r] = (ld)xyz[r] - (ld)v[0][r];
+            }
+            auto det3 = [](ld M[3][3]) {
+                return M[0][0] * (M[1][1] * M[2][2] - M[1][2] * M[2][1]) - M[0][1] * (M[1][0] * M[2][2] - M[1][2] * M[2][0]) +
+                       M[0][2] * (M[1][0] * M[2][1] - M[1][1] * M[2][0]);
+            };
+            const ld D = det3(A);
+            ld l[4];
+            l[0] = 1;
+            for (int c = 0; c < 3; ++c) {
+                ld B[3][3];
+                for (int r = 0; r < 3; ++r)
+                    for (int q = 0; q < 3; ++q) B[r][q] = q == c ? b[r] : A[r][q];
+                l[c + 1] = det3(B) / D;
+                l[0] -= l[c + 1];
+            }
+            if (std::min(std::min(l[0], l[1]), std::min(l[2], l[3])) >= -1e-12L) {
+                kfound = k;
+                for (int i = 0; i < 4; ++i) lam[i] = l[i];
+            }
+        }
+        if (kfound < 0) throw std::runtime_error("EINVAL: the source point is outside the mesh");
+        const ld rst[3] = {-1 + 2 * lam[1], -1 + 2 * lam[2], -1 + 2 * lam[3]};
+        std::vector<double> w = dg::delta_weights(m.r3, rst);
+        for (double& x : w) x /= m.J3[kfound];
+        cu(cudaStreamSynchronize(s->stream), "sync");
+        if (s->precision == 64) {
+            cu(cudaMemcpy(s->src_w, w.data(), sizeof(double) * w.size(), cudaMemcpyHostToDevice), "upload weights");
+        } else {
+            std::vector<float> wf(w.begin(), w.end());
+            cu(cudaMemcpy(s->src_w, wf.data(), sizeof(float) * wf.size(), cudaMemcpyHostToDevice), "upload weights");
+        }
+        s->src_k = kfound; s->src_f = f_peak; s->src_ts = t_s; s->src_amp = amplitude;
+        s->src_on = amplitude != 0.0;
+        for (int i = 0; i < 2; ++i)                 // the captured step no longer matches
+            if (s->graph[i]) { cudaGraphExecDestroy(s->graph[i]); s->graph[i] = nullptr; }
         return DG_OK;
     } catch (const std::exception& e) { return err_from_exception(e); }
 }

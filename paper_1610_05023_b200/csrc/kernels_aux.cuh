@@ -387,6 +387,27 @@ __global__ void k_close_corner(Dev<T> d, int cur) {
     }
 }
 
+// Point source delta(x - xs) S(t) in the pressure equation (S = integral of the Ricker wavelet (44)).
+// Runs right after the 3D kernel of a stage: the fused kernel has applied res = a res + dt F, q += b res, and F
+// is linear in the source, so the source's share is res_p += dt f, q_p += b dt f on the nodes of the source cell.
+// The simulated time lives on the device (the step is replayed as a CUDA graph): *t_dev is the time at the start of
+// the step, the last stage's launch advances it.
+template <typename T>
+__global__ void k_source(T* __restrict__ qnew, T* __restrict__ res, const T* __restrict__ w, int k, int Np, double* t_dev,
+                         double rkc_dt, double dt, double rkb, double fpeak, double ts, double amp, int last) {
+    const double t = *t_dev + rkc_dt;
+    __syncthreads();
+    const double tau = t - ts, a = 3.14159265358979323846 * fpeak * tau;
+    const double S = amp * tau * exp(-a * a);
+    for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+        const double f = S * (double)w[n];
+        const size_t o = ((size_t)k * Np + n) * 4;
+        res[o] = (T)((double)res[o] + dt * f);
+        qnew[o] = (T)((double)qnew[o] + rkb * dt * f);
+    }
+    if (last && threadIdx.x == 0) *t_dev = *t_dev + dt;
+}
+
 // dg_set_initial / dg_get_fields: interface arrays are fp64 [K][Np] per field; the device state is [K][Np][4] of T
 template <typename T>
 __global__ void k_pack_field(const double* __restrict__ stage, T* __restrict__ q, int fld, size_t n) {

@@ -258,6 +258,21 @@ static std::vector<ld> matmul(const std::vector<ld>& A, const std::vector<ld>& B
     return C;
 }
 
+// (M^-1 l(x))_n = sum_m V_nm psi_m(x): the Galerkin weights of a Dirac delta at reference point x
+std::vector<double> delta_weights(const RefElem& e, const ld* x) {
+    std::vector<ld> V, Vx, G[3], Gx[3];
+    vandermonde(e.dim, e.N, e.rst, e.Np, V, G);
+    std::vector<ld> xs(x, x + e.dim);
+    vandermonde(e.dim, e.N, xs, 1, Vx, Gx);
+    std::vector<double> w(e.Np);
+    for (int n = 0; n < e.Np; ++n) {
+        ld s = 0;
+        for (int m = 0; m < e.Np; ++m) s += V[(size_t)n * e.Np + m] * Vx[m];
+        w[n] = (double)s;
+    }
+    return w;
+}
+
 RefElem make_refelem(int dim, int N) {
     if (dim < 1 || dim > 3 || N < 1 || N > 8) throw std::runtime_error("make_refelem: need dim in 1..3, N in 1..8");
     RefElem e;

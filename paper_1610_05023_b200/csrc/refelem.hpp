@@ -36,6 +36,9 @@ extern const int TRI_NHAT[3][2];
 
 RefElem make_refelem(int dim, int N);
 
+// Weights (M^-1 l(x))_n of a Dirac delta at the reference point x[dim] (point source).
+std::vector<double> delta_weights(const RefElem& e, const ld* x);
+
 // Dense helpers shared by the host setup (long double Gauss-Jordan inverse with partial pivoting).
 std::vector<ld> invert(const std::vector<ld>& A, int n);
 

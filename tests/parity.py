@@ -33,25 +33,29 @@ def initial_on(w, x, y, z, c_elem, rho_elem):
     return w.fields(x, y, z, cn, rn)
 
 
-def run_oracle(w, nsteps=None, dt=None, face_bc=None):
+def run_oracle(w, nsteps=None, dt=None, face_bc=None, source=None):
     from oracle.solver import OracleSolver
     face_bc = getattr(w, "face_bc", None) if face_bc is None else face_bc
     o = OracleSolver(w.verts, w.tets, w.N, w.J, w.c, w.rho, dt=dt, face_bc=face_bc)
     x = o.nodes()
     o.set_initial(np.stack(initial_on(w, x[..., 0], x[..., 1], x[..., 2], w.c, w.rho)))
+    if source:
+        o.set_source(*source)                    # (xs, f_peak, t_s, amplitude)
     o.step(w.nsteps if nsteps is None else nsteps)
     q, fa, ea = o.get_fields()
     return dict(dt=o.dt, x=x, q=q, fa=fa, ea=ea, xf=o.H.tri.x if o.T else np.zeros((0, 1, 3)),
                 xe=o.H.lin.x if o.E else np.zeros((0, 1, 3)), T=o.T, E=o.E, C=o.C)
 
 
-def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True, kernel=0, face_bc=None):
+def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True, kernel=0, face_bc=None, source=None):
     from paper_1610_05023_b200 import Solver
     face_bc = getattr(w, "face_bc", None) if face_bc is None else face_bc
     s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=precision, dt=dt, use_graph=use_graph, kernel=kernel,
                face_bc=face_bc)
     x, y, z = s.get_nodes()
     s.set_initial(*initial_on(w, x, y, z, w.c, w.rho))
+    if source:
+        s.set_source(*source)
     s.step(w.nsteps if nsteps is None else nsteps)
     q, fa, ea = s.get_fields()
     _, _, _, _, xf = s.get_face_map()

@@ -135,6 +135,54 @@ def test_seam_shaped_workload(prec):
     _check(parity.compare(lib, ora), prec)
 
 
+@pytest.mark.parametrize("N,prec,kernel,graph", [(3, 64, 0, True), (5, 64, 0, True), (4, 64, 1, False), (5, 32, 0, True), (2, 32, 0, True)])
+def test_point_source(N, prec, kernel, graph):
+    """Ricker point source in the pressure equation on top of the seeded pulse, against
+    the oracle; the source cell is strictly inside the mesh and the stage times t + c_n dt matter (S changes sign)."""
+    w = make_workload("cfg1", n=3, N=N, J=2, nsteps=40)
+    src = ([0.11, -0.07, 0.05], 2.5, 0.05, 3.0)
+    lib = parity.run_library(w, precision=prec, kernel=kernel, use_graph=graph, source=src)
+    ora = parity.run_oracle(w, source=src)
+    nosrc = parity.run_oracle(w)
+    assert parity.rel_l2(ora["q"], nosrc["q"]) > 0.05                # the source really contributes
+    _check(parity.compare(lib, ora), prec)
+    assert lib["info"]["launches_per_step"] == 35
+
+
+def test_point_source_spherical_wave_and_reset():
+    """The CUDA path against the analytic spherical wave (45a-b) at a resolution the oracle would need minutes for
+    (12^3 x 6 tets, N = 4), and dg_set_initial restarting the clock / amplitude 0 switching the source off."""
+    from paper_1610_05023_b200 import Solver
+    from workloads.configs import box_mesh
+    v, t = box_mesh((12, 12, 12), ((-0.5, 0.5),) * 3)
+    K = len(t)
+    xs, f, ts = np.array([0.03, 0.02, 0.01]), 2.5, 0.5
+    s = Solver(v, t, 4, 4, np.ones(K), np.ones(K))
+    x, y, z = s.get_nodes()
+    zero = np.zeros_like(x)
+
+    def solve(amplitude):
+        s.set_initial(zero, zero, zero, zero)
+        s.set_source(xs, f, ts, amplitude)
+        nst = int(round(0.9 / s.dt))
+        s.step(nst)
+        return s.get_fields(aux=False)[0], nst * s.dt
+
+    q, tf = solve(1.0)
+    d = np.stack([x, y, z], axis=-1) - xs
+    r = np.linalg.norm(d, axis=-1)
+    a = (np.pi * f * (tf - r - ts)) ** 2
+    pref = (1.0 - 2.0 * a) * np.exp(-a) / (4.0 * np.pi * r)
+    m = r > 0.15
+    err = np.linalg.norm((q[0] - pref)[m]) / np.linalg.norm(pref[m])
+    assert err < 0.02, err
+    q2, _ = solve(1.0)                                               # same answer after a restart: the clock was reset
+    assert np.abs(q2 - q).max() <= 1e-13 * np.abs(q).max()
+    q0, _ = solve(0.0)
+    assert not q0.any()
+    s.close()
+
+
 def test_edge_cases():
     """Smallest mesh (one hex, 6 tets: every tet touches the boundary), J=1, J=12 (maximum), graph off,
     negatively oriented input cells, zero initial data, nsteps=0."""
