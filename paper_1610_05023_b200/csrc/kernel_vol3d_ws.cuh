@@ -36,7 +36,11 @@ struct WsCfg {
     static constexpr int LPAD = KPL * EB + 8;          // stride of one face block of the flux operand (bank spread)
     static constexpr int NT = 384;
     static constexpr int NS = 3;                       // staging depth
-    static constexpr int QS = Np * 4 + 2;              // staged element stride of q / res (16 B skew)
+    // staged q / res: element e sits at e * QS + 2 * slot(e) doubles, QS a multiple of 128 bytes and slot(e) a
+    // permutation of the eight 16-byte bank groups chosen so that BOTH access patterns are conflict-free: PREP
+    // (8 elements, one node per quarter-warp) and the update of the MMA warps (4 elements of equal parity x 2
+    // adjacent nodes per quarter-warp: elements {0,2,4,6} -> slots {0,1,4,5}, {1,3,5,7} -> {2,3,6,7})
+    static constexpr int QS = ((Np * 4 + 15) / 16) * 16 + 16;
     static constexpr int GS = GX3 + 2;                 // staged stride of the geometric record: 336 B, so that the
                                                        // records of elements 0,2,4,6 (and 0..7) fall in distinct banks
     static constexpr int szB = 4 * KPD * EB + 4 * LPAD;
@@ -57,6 +61,11 @@ struct WsCfg {
     static_assert((REG_BASE - REG_PREP) * 128 >= (REG_MMA - REG_BASE) * 256, "setmaxnreg pool would deadlock");
     static_assert(MT <= 7, "the warp-specialised kernel covers N <= 5");
 };
+
+__device__ __forceinline__ int ws_eoff(int e, int QS) {
+    const int a = e >> 1;
+    return e * QS + 2 * (2 * (e & 1) + (a & 1) + 4 * (a >> 1));
+}
 
 __device__ __forceinline__ double2 ldg_nc2(const double* p) {
     double2 v;
@@ -125,7 +134,7 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
         int it = 0;
         for (int b = blockIdx.x; b < nbatch; b += gridDim.x, ++it) {
             const int s = it % NS, o = it & 1;
-            const double* bq = sQ + (s * EB + ie) * QS;
+            const double* bq = sQ + s * EB * QS + ws_eoff(ie, QS);
             const double* ge = sGeo + (s * EB + ie) * GS;
             const double* bn = sN + s * (Nfn * EB * 4) + f * (Nfp * 32) + ie * 4;
             const int h0 = 2 * ((ie >> 2) & 1);
@@ -194,8 +203,8 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
             const size_t e0 = (size_t)b * EB;
             if (lane == 0) mbar_arrive_expect_tx(&full[s], C::tx_bytes);
             __syncwarp();
-            if (lane < EB) bulk_g2s(sQ + (s * EB + lane) * QS, qold + (e0 + lane) * (Np * 4), Np * 32, &full[s]);
-            else if (lane < 2 * EB) bulk_g2s(sR + (s * EB + lane - EB) * QS, d.res + (e0 + lane - EB) * (Np * 4), Np * 32, &full[s]);
+            if (lane < EB) bulk_g2s(sQ + s * EB * QS + ws_eoff(lane, QS), qold + (e0 + lane) * (Np * 4), Np * 32, &full[s]);
+            else if (lane < 2 * EB) bulk_g2s(sR + s * EB * QS + ws_eoff(lane - EB, QS), d.res + (e0 + lane - EB) * (Np * 4), Np * 32, &full[s]);
             else if (lane < 3 * EB) bulk_g2s(sGeo + (s * EB + lane - 2 * EB) * GS, geox + (e0 + lane - 2 * EB) * GX3, GX3 * 8, &full[s]);
             // neighbour traces (16-byte cp.async gathers), or the ghost state (2 r^-, 0, 0, 0) behind an HABC face;
             // this half-warp serves faces 2 hw and 2 hw + 1 of element ie
@@ -307,10 +316,11 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
                     const double ru = g01.x * xr + g23.y * xs + g67.x * xt;
                     const double rv = g01.y * xr + g45.x * xs + g67.y * xt;
                     const double rw = g23.x * xr + g45.y * xs + g8r.x * xt;
-                    double2 q0 = *reinterpret_cast<const double2*>(bq + e * QS + n * 4);
-                    double2 q1 = *reinterpret_cast<const double2*>(bq + e * QS + n * 4 + 2);
-                    double2 r0 = *reinterpret_cast<const double2*>(br + e * QS + n * 4);
-                    double2 r1 = *reinterpret_cast<const double2*>(br + e * QS + n * 4 + 2);
+                    const int eo = ws_eoff(e, QS) + n * 4;
+                    double2 q0 = *reinterpret_cast<const double2*>(bq + eo);
+                    double2 q1 = *reinterpret_cast<const double2*>(bq + eo + 2);
+                    double2 r0 = *reinterpret_cast<const double2*>(br + eo);
+                    double2 r1 = *reinterpret_cast<const double2*>(br + eo + 2);
                     r0.x = rka * r0.x + rp;  q0.x += rkb * r0.x;
                     r0.y = rka * r0.y + ru;  q0.y += rkb * r0.y;
                     r1.x = rka * r1.x + rv;  q1.x += rkb * r1.x;
