@@ -47,7 +47,7 @@ __host__ __device__ inline int face2d_ops_elems(int Nfp, int N1) {          // o
 #endif
 template <typename T>
 __global__ void __launch_bounds__(FACE2D_NT, FACE2D_MINB) k_face2d(Dev<T> d, int src, T rka, T rkb, T dt) {
-    extern __shared__ __align__(32) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int SB = FACE2D_SB;
     const int Nfp = d.Nfp, N1 = d.N1, J = d.J, Nf = 3 * d.N1;
     const int W = max(Nfp, Nf);                   // thread slots per item (3 N1 > Nfp for N <= 3)
@@ -229,7 +229,7 @@ __device__ __forceinline__ T edge_pressure(const Dev<T>& d, const T* ea, int ell
 
 template <typename T>
 __global__ void k_edge1d(Dev<T> d, int src, T rka, T rkb, T dt) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     const int J = d.J, N1 = d.N1, JJ = J * J;
     T* sp = reinterpret_cast<T*>(smem_raw);       // [JJ][N1]
     T* sw = sp + JJ * N1;
@@ -363,7 +363,7 @@ __global__ void __launch_bounds__(32 * CLOSE_EDGE_WARPS) k_close_edge(Dev<T> d, 
 // independent), shuffle reduction.
 template <typename T>
 __global__ void k_close_corner(Dev<T> d, int cur) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     T* srp = reinterpret_cast<T*>(smem_raw);      // [3 J^2]
     const int J = d.J, JJ = J * J, N1 = d.N1, c = blockIdx.x, n3 = 3 * JJ;
     for (int r = threadIdx.x; r < n3; r += blockDim.x) {
