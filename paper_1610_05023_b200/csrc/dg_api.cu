@@ -345,6 +345,28 @@ void launch_vol3d_cfg(dg_solver* s, Dev<T>& d, int src, double a, double b, bool
     kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
 }
 
+template <typename T, int N, int NB, int ET, int G>
+void launch_vol3d_rb_cfg(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
+    using Cfg = Vol3dRbCfg<T, N, NB, ET, G>;
+    auto kern = k_vol3d_rb<T, N, NB, ET, G>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int per_sm = 0, sms = 0;
+        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: register-blocked volume kernel does not fit on an SM");
+        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
+        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
+}
+
+// register blocking of k_vol3d_rb, from the sweep in profiles/r02_degree_sweep.md (fp64: 3 elements per warp, fp32: 4)
+template <typename T> struct RbEt { static constexpr int value = 3; };
+template <> struct RbEt<float> { static constexpr int value = 4; };
+
 template <typename T> struct OpsFit;
 template <> struct OpsFit<double> { static constexpr int maxN = 5; };
 template <> struct OpsFit<float> { static constexpr int maxN = 6; };
@@ -492,9 +514,19 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool con
         case 3: launch_vol3d_cfg<T, 3, 8, 4, true>(s, d, src, a, b, configure); break;
         case 4: launch_vol3d_cfg<T, 4, 8, 4, true>(s, d, src, a, b, configure); break;
         case 5: launch_vol3d_cfg<T, 5, 4, 4, true>(s, d, src, a, b, configure); break;
-        case 6: launch_vol3d_cfg<T, 6, 4, 2, (6 <= mx)>(s, d, src, a, b, configure); break;
-        case 7: launch_vol3d_cfg<T, 7, 2, 4, false>(s, d, src, a, b, configure); break;
-        case 8: launch_vol3d_cfg<T, 8, 2, 2, false>(s, d, src, a, b, configure); break;
+        case 6:
+            if (s->kernel == 1) launch_vol3d_cfg<T, 6, 4, 2, (6 <= mx)>(s, d, src, a, b, configure);
+            else launch_vol3d_rb_cfg<T, 6, 3, RbEt<T>::value, 4>(s, d, src, a, b, configure);
+            break;
+        case 7:
+            if (s->kernel == 1) launch_vol3d_cfg<T, 7, 2, 4, false>(s, d, src, a, b, configure);
+            else launch_vol3d_rb_cfg<T, 7, 4, RbEt<T>::value, 4>(s, d, src, a, b, configure);
+            break;
+        case 8:
+            // fp64, N = 8: the register-blocked kernel (182 registers at 2 elements per warp) is not faster
+            if (s->kernel == 1 || std::is_same<T, double>::value) launch_vol3d_cfg<T, 8, 2, 2, false>(s, d, src, a, b, configure);
+            else launch_vol3d_rb_cfg<T, 8, 6, 2, 4>(s, d, src, a, b, configure);
+            break;
         default: throw std::runtime_error("EINVAL: N must be in 1..8");
     }
 }

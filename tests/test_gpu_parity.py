@@ -71,7 +71,7 @@ def test_J8_degree(N):
         _check(parity.compare(lib, ora), prec)
 
 
-@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (4, 4), (4, 6), (5, 1), (5, 2), (5, 3), (5, 4), (5, 6), (2, 2)])
+@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (4, 4), (4, 6), (5, 1), (5, 2), (5, 3), (5, 4), (5, 6), (2, 2), (6, 1), (6, 0), (7, 1)])
 def test_3d_kernel_variants(N, kernel):
     """dg_options.kernel: 1 scalar FMA, 2 batch-synchronous DMMA, 3 warp-specialised DMMA, 4 the same with the update in
     its own warpgroup -- the same numbers.
