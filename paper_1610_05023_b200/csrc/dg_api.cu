@@ -20,6 +20,7 @@
 #include "kernel_vol3d_ws2.cuh"
 #include "kernel_vol3d_wsp.cuh"
 #include "kernel_vol3d_tf32.cuh"
+#include "kernel_vol3d_mmag.cuh"
 #include "mesh.hpp"
 
 namespace {
@@ -82,6 +83,7 @@ struct dg_solver {
     int kernel = 0;                 // dg_options.kernel as requested
     bool mma3 = false;              // the tensor-pipe 3D kernel is in use
     bool ws3 = false;               // ... in its warp-specialised form (kernel_vol3d_ws.cuh)
+    bool mmag = false;              // fp64, N >= 6: tensor-pipe kernel with the operators read through L1/L2 (kernel_vol3d_mmag.cuh)
     bool ws6 = false;               // ... with the software-pipelined MMA loop (kernel_vol3d_wsp.cuh); implies ws3
     bool ws4 = false;               // ... with the update in its own warpgroup (kernel_vol3d_ws2.cuh); implies ws3
     const void* geox3 = nullptr;    // [Kp][GX3] per-tet record of the warp-specialised kernels (dt folded in), fp64 or fp32
@@ -363,6 +365,37 @@ void launch_vol3d_rb_cfg(dg_solver* s, Dev<T>& d, int src, double a, double b, b
     kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
 }
 
+#ifndef MMAG_NTILE
+#define MMAG_NTILE 2
+#endif
+#ifndef MMAG_W6
+#define MMAG_W6 8
+#endif
+#ifndef MMAG_W7
+#define MMAG_W7 8
+#endif
+#ifndef MMAG_W8
+#define MMAG_W8 8
+#endif
+template <int N>
+void launch_vol3d_mmag_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    constexpr int MMAG_W = N == 6 ? MMAG_W6 : N == 7 ? MMAG_W7 : MMAG_W8;
+    using Cfg = MmagCfg<N, MMAG_NTILE, MMAG_W>;
+    auto kern = k_vol3d_mmag<N, MMAG_NTILE, MMAG_W>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int per_sm = 0, sms = 0;
+        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: tensor-pipe volume kernel (N >= 6) does not fit on an SM");
+        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
+        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, a, b, s->dt);
+}
+
 // register blocking of k_vol3d_rb, from the sweep in profiles/r02_degree_sweep.md (fp64: 3 elements per warp, fp32: 4)
 template <typename T> struct RbEt { static constexpr int value = 3; };
 template <> struct RbEt<float> { static constexpr int value = 4; };
@@ -502,6 +535,16 @@ void launch_vol3d_tf32(dg_solver* s, Dev<float>& d, int src, double a, double b,
 template <typename T>
 void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
     constexpr int mx = OpsFit<T>::maxN;
+    if constexpr (std::is_same<T, double>::value) {
+        if (s->mmag) {
+            switch (s->N) {
+                case 6: return launch_vol3d_mmag_cfg<6>(s, d, src, a, b, configure);
+                case 7: return launch_vol3d_mmag_cfg<7>(s, d, src, a, b, configure);
+                case 8: return launch_vol3d_mmag_cfg<8>(s, d, src, a, b, configure);
+                default: break;
+            }
+        }
+    }
     if constexpr (std::is_same<T, float>::value) {
         if (s->tf3) return launch_vol3d_tf32(s, d, src, a, b, configure);
     }
@@ -523,8 +566,7 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool con
             else launch_vol3d_rb_cfg<T, 7, 4, RbEt<T>::value, 4>(s, d, src, a, b, configure);
             break;
         case 8:
-            // fp64, N = 8: the register-blocked kernel (182 registers at 2 elements per warp) is not faster
-            if (s->kernel == 1 || std::is_same<T, double>::value) launch_vol3d_cfg<T, 8, 2, 2, false>(s, d, src, a, b, configure);
+            if (s->kernel == 1) launch_vol3d_cfg<T, 8, 2, 2, false>(s, d, src, a, b, configure);
             else launch_vol3d_rb_cfg<T, 8, 6, 2, 4>(s, d, src, a, b, configure);
             break;
         default: throw std::runtime_error("EINVAL: N must be in 1..8");
@@ -823,7 +865,10 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
         s->use_graph = opt ? opt->use_graph != 0 : true;
         s->kernel = opt ? opt->kernel : 0;
-        if (s->kernel < 0 || s->kernel > 6) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..6");
+        if (s->kernel < 0 || s->kernel > 8) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..8");
+        if (s->kernel == 8 && N < 6) throw std::runtime_error("EINVAL: kernel = 8 covers N = 6..8");
+        if (s->kernel == 7 && (precision != 64 || N < 6))
+            throw std::runtime_error("EINVAL: kernel = 7 covers fp64, N = 6..8");
         if (s->kernel == 5 && (precision != 32 || N < TF32_MIN_N || N > TF32_MAX_N))
             throw std::runtime_error("EINVAL: the fp32 tensor-core kernel (kernel = 5) covers fp32, N = 3..5");
         if ((s->kernel == 3 || s->kernel == 4 || s->kernel == 6) && (precision != 64 || N < 4 || N > 5))
@@ -833,6 +878,7 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         if (mesh->ntets > CONN_MAX_ID) throw std::runtime_error("EINVAL: more than 2^26 - 1 tetrahedra");
         s->mma3 = precision == 64 && N <= MMA_MAX_N && s->kernel != 1;
         s->tf3 = precision == 32 && N >= TF32_MIN_N && N <= TF32_MAX_N && (s->kernel == 0 || s->kernel == 5);
+        s->mmag = precision == 64 && N >= 6 && (s->kernel == 0 || s->kernel == 7);
         s->ws4 = s->mma3 && s->kernel == 4;
         s->ws6 = s->mma3 && s->kernel == 6;
         s->ws3 = s->mma3 && (s->ws4 || s->ws6 || s->kernel == 3 || (s->kernel == 0 && N == 5));

@@ -71,10 +71,11 @@ def test_J8_degree(N):
         _check(parity.compare(lib, ora), prec)
 
 
-@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (4, 4), (4, 6), (5, 1), (5, 2), (5, 3), (5, 4), (5, 6), (2, 2), (6, 1), (6, 0), (7, 1)])
+@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (4, 4), (4, 6), (5, 1), (5, 2), (5, 3), (5, 4), (5, 6), (2, 2), (6, 1), (6, 0), (7, 1), (6, 8), (7, 8), (8, 8), (8, 0)])
 def test_3d_kernel_variants(N, kernel):
     """dg_options.kernel: 1 scalar FMA, 2 batch-synchronous DMMA, 3 warp-specialised DMMA, 4 the same with the update in
-    its own warpgroup -- the same numbers.
+    its own warpgroup, 6 software-pipelined; N >= 6: 0/7 tensor pipe with operators from L1/L2, 8 register-blocked
+    scalar -- the same numbers.
     5^3 hexes = 750 tets: 93 batches of 8 + a ragged tail of 6, several batches per persistent CTA."""
     w = make_workload("cfg5", n=5, N=N, J=3, nsteps=12)
     lib, ora = parity.run_library(w, kernel=kernel), parity.run_oracle(w)
