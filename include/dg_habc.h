@@ -61,8 +61,8 @@ typedef struct {
                                  (the choice at N = 5); 4 = experimental variant of 3 with the update in helper
                                  warps; 6 = experimental variant of 3 with a software-pipelined MMA loop;
                                  5 = fp32 tensor-core kernel (3xTF32, fp32-accurate), N = 3..5 (the choice there);
-                                 7 = fp64 tensor-pipe kernel with the operators read through L1/L2, N = 6..8 (the
-                                 choice there); 8 = register-blocked scalar kernel, N = 6..8 (the choice in fp32).  A kernel that does not cover (N, precision) gives DG_EINVAL */
+                                 7 = tensor-pipe kernels with the operators read through L1/L2, N = 6..8 (fp64 DMMA /
+                                 fp32 3xTF32; the choice there); 8 = register-blocked scalar kernel, N = 6..8.  A kernel that does not cover (N, precision) gives DG_EINVAL */
     int32_t face_bc[6];       /* boundary condition of the six domain faces, index axis * 2 + (1 for the face at the upper
                                  end of the axis): 0 = HABC (the default), 1 = p = 0 (free surface),
                                  2 = rigid wall (n.u = 0).  Auxiliary fields exist only on HABC faces, on the edges

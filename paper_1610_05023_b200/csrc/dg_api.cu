@@ -21,6 +21,7 @@
 #include "kernel_vol3d_wsp.cuh"
 #include "kernel_vol3d_tf32.cuh"
 #include "kernel_vol3d_mmag.cuh"
+#include "kernel_vol3d_tf32g.cuh"
 #include "mesh.hpp"
 
 namespace {
@@ -83,6 +84,7 @@ struct dg_solver {
     int kernel = 0;                 // dg_options.kernel as requested
     bool mma3 = false;              // the tensor-pipe 3D kernel is in use
     bool ws3 = false;               // ... in its warp-specialised form (kernel_vol3d_ws.cuh)
+    bool tfg = false;               // fp32, N >= 6: 3xTF32 tensor-core kernel with the operators read through L1/L2
     bool mmag = false;              // fp64, N >= 6: tensor-pipe kernel with the operators read through L1/L2 (kernel_vol3d_mmag.cuh)
     bool ws6 = false;               // ... with the software-pipelined MMA loop (kernel_vol3d_wsp.cuh); implies ws3
     bool ws4 = false;               // ... with the update in its own warpgroup (kernel_vol3d_ws2.cuh); implies ws3
@@ -396,6 +398,25 @@ void launch_vol3d_mmag_cfg(dg_solver* s, Dev<double>& d, int src, double a, doub
     kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, a, b, s->dt);
 }
 
+template <int N>
+void launch_vol3d_tf32g_cfg(dg_solver* s, Dev<float>& d, int src, double a, double b, bool configure) {
+    constexpr int TFG_W = N == 6 ? 7 : N == 7 ? 8 : 11;     // warps per CTA, from the sweep in profiles/r02_degree_sweep.md
+    using Cfg = TfgCfg<N, TFG_W>;
+    auto kern = k_vol3d_tf32g<N, TFG_W>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int per_sm = 0, sms = 0;
+        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: fp32 tensor-core volume kernel (N >= 6) does not fit on an SM");
+        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
+        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (float)a, (float)b, (float)s->dt);
+}
+
 // register blocking of k_vol3d_rb, from the sweep in profiles/r02_degree_sweep.md (fp64: 3 elements per warp, fp32: 4)
 template <typename T> struct RbEt { static constexpr int value = 3; };
 template <> struct RbEt<float> { static constexpr int value = 4; };
@@ -547,6 +568,14 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool con
     }
     if constexpr (std::is_same<T, float>::value) {
         if (s->tf3) return launch_vol3d_tf32(s, d, src, a, b, configure);
+        if (s->tfg) {
+            switch (s->N) {
+                case 6: return launch_vol3d_tf32g_cfg<6>(s, d, src, a, b, configure);
+                case 7: return launch_vol3d_tf32g_cfg<7>(s, d, src, a, b, configure);
+                case 8: return launch_vol3d_tf32g_cfg<8>(s, d, src, a, b, configure);
+                default: break;
+            }
+        }
     }
     if constexpr (std::is_same<T, double>::value) {
         if (s->mma3) return launch_vol3d_mma(s, d, src, a, b, configure);
@@ -867,8 +896,7 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->kernel = opt ? opt->kernel : 0;
         if (s->kernel < 0 || s->kernel > 8) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..8");
         if (s->kernel == 8 && N < 6) throw std::runtime_error("EINVAL: kernel = 8 covers N = 6..8");
-        if (s->kernel == 7 && (precision != 64 || N < 6))
-            throw std::runtime_error("EINVAL: kernel = 7 covers fp64, N = 6..8");
+        if (s->kernel == 7 && N < 6) throw std::runtime_error("EINVAL: kernel = 7 covers N = 6..8");
         if (s->kernel == 5 && (precision != 32 || N < TF32_MIN_N || N > TF32_MAX_N))
             throw std::runtime_error("EINVAL: the fp32 tensor-core kernel (kernel = 5) covers fp32, N = 3..5");
         if ((s->kernel == 3 || s->kernel == 4 || s->kernel == 6) && (precision != 64 || N < 4 || N > 5))
@@ -879,6 +907,7 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->mma3 = precision == 64 && N <= MMA_MAX_N && s->kernel != 1;
         s->tf3 = precision == 32 && N >= TF32_MIN_N && N <= TF32_MAX_N && (s->kernel == 0 || s->kernel == 5);
         s->mmag = precision == 64 && N >= 6 && (s->kernel == 0 || s->kernel == 7);
+        s->tfg = precision == 32 && N >= 6 && (s->kernel == 0 || s->kernel == 7);
         s->ws4 = s->mma3 && s->kernel == 4;
         s->ws6 = s->mma3 && s->kernel == 6;
         s->ws3 = s->mma3 && (s->ws4 || s->ws6 || s->kernel == 3 || (s->kernel == 0 && N == 5));

@@ -82,16 +82,17 @@ def test_3d_kernel_variants(N, kernel):
     _check(parity.compare(lib, ora), 64)
 
 
-@pytest.mark.parametrize("N,kernel", [(3, 5), (4, 5), (5, 5), (3, 1), (5, 1), (5, 0)])
+@pytest.mark.parametrize("N,kernel", [(3, 5), (4, 5), (5, 5), (3, 1), (5, 1), (5, 0), (6, 7), (7, 7), (8, 7), (6, 0), (6, 8)])
 def test_3d_kernel_variants_fp32(N, kernel):
-    """fp32: 1 scalar FMA, 5 tensor cores with 3xTF32 error compensation (the default for N = 3..5) -- both inside the
+    """fp32: 1 scalar FMA, 5 / 7 tensor cores with 3xTF32 error compensation (N = 3..5 / N = 6..8), 8 register-blocked
+    FMA -- all inside the
     fp32 tolerance, and the compensated tensor-core result no worse than 4x the FMA kernel's error.
     750 tets = 46 batches of 16 + a ragged tail of 14."""
     w = make_workload("cfg5", n=5, N=N, J=3, nsteps=12)
     ora = parity.run_oracle(w)
     err = parity.compare(parity.run_library(w, precision=32, kernel=kernel), ora)
     _check(err, 32)
-    if kernel == 5:
+    if kernel in (5, 7):
         ref = parity.compare(parity.run_library(w, precision=32, kernel=1), ora)
         assert err["p"] <= 4 * ref["p"] + 1e-7 and err["u"] <= 4 * ref["u"] + 1e-7, (err, ref)
 
