@@ -105,14 +105,21 @@ k_vol3d_mmag(Dev<double> d, int src, double rka, double rkb, double dt) {
 #pragma unroll
                 for (int v = 0; v < 10; ++v) acc[q][v][0] = acc[q][v][1] = 0.0;
             const double* bp = sB + t * 8 + (g ^ swz(t));
-#pragma unroll 2
-            for (int s_ = 0; s_ < KD; ++s_) {
+            // operator fragments one k-step ahead: their L1/L2 latency is the cost of this kernel
+            auto loadD = [&](int s_, double& ar, double& as, double& at) {
                 const int m = 4 * s_ + t;
                 const bool ok = nok && m < Np;
                 const int mc = min(m, Np - 1);
-                const double ar = ok ? d.Dt3[(0 * Np + mc) * Np + nc] : 0.0;     // Dt3[a][m][n] = D_a[n][m]
-                const double as = ok ? d.Dt3[(1 * Np + mc) * Np + nc] : 0.0;
-                const double at = ok ? d.Dt3[(2 * Np + mc) * Np + nc] : 0.0;
+                ar = ok ? d.Dt3[(0 * Np + mc) * Np + nc] : 0.0;                 // Dt3[a][m][n] = D_a[n][m]
+                as = ok ? d.Dt3[(1 * Np + mc) * Np + nc] : 0.0;
+                at = ok ? d.Dt3[(2 * Np + mc) * Np + nc] : 0.0;
+            };
+            double ar, as, at;
+            loadD(0, ar, as, at);
+#pragma unroll 2
+            for (int s_ = 0; s_ < KD; ++s_) {
+                double nr, ns, nt_;
+                loadD(min(s_ + 1, KD - 1), nr, ns, nt_);
 #pragma unroll
                 for (int q = 0; q < NTILE; ++q) {
                     const double* b = bp + q * szT + (4 * s_) * 8;
@@ -124,6 +131,7 @@ k_vol3d_mmag(Dev<double> d, int src, double rka, double rkb, double dt) {
                     dmma884(acc[q][4], as, b[2 * KPD * 8]);
                     dmma884(acc[q][5], at, b[3 * KPD * 8]);
                 }
+                ar = nr; as = ns; at = nt_;
             }
             for (int s_ = 0; s_ < KL; ++s_) {
                 const int j = 4 * s_ + t;
