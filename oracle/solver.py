@@ -17,7 +17,7 @@ from . import habc
 from .mesh import BC_DIRICHLET, BC_HABC, BC_INT, BC_RIGID, Hierarchy, Level, build_hierarchy
 
 # LSRK4(5) of Carpenter & Kennedy, ref. [10] of the paper (coefficients not printed there,
-# pinned by the order conditions in tests/test_oracle_lsrk.py)
+# pinned by the order conditions in tests/test_oracle_refelem_habc.py::test_lsrk_order_conditions)
 RK4A = np.array([0.0,
                  -567301805773.0 / 1357537059087.0,
                  -2404267990393.0 / 2016746695238.0,
