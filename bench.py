@@ -213,12 +213,7 @@ def main():
     alu["frac"] = alu["achieved"] / alu["peak"]
     t_mem, t_alu = bytes_launch / (hbm_peak * 1e9), flops_launch / (alu_peak * 1e12)
     roof = dict(hbm if t_mem >= t_alu else alu)
-    if prec == 64:
-        kname = {0: "k_vol3d_ws" if w.N == 5 else "k_vol3d_mma" if w.N < 5 else "k_vol3d_mmag", 1: "k_vol3d", 7: "k_vol3d_mmag", 8: "k_vol3d_rb", 2: "k_vol3d_mma",
-                 3: "k_vol3d_ws", 4: "k_vol3d_ws2", 6: "k_vol3d_wsp"}.get(args.kernel, "k_vol3d")
-    else:
-        kname = "k_vol3d_tf32" if 3 <= w.N <= 5 and args.kernel in (0, 5) else "k_vol3d_tf32g" if w.N >= 6 and args.kernel in (0, 7) else "k_vol3d_rb" if w.N >= 6 and args.kernel == 8 else "k_vol3d"
-    roof.update({"kernel": f"{kname}<{w.N}>", "ms_per_launch": vol_ms, "traffic": None,
+    roof.update({"kernel": s.info["kernel_name"], "ms_per_launch": vol_ms, "traffic": None,
                  "roof_ms": 1e3 * max(t_mem, t_alu), "frac_of_slower_roof": max(t_mem, t_alu) / (vol_ms * 1e-3),
                  "hbm": hbm, "alu": alu, "kernel_share_of_step": prof["vol3d"] / max(sum(prof.values()), 1e-12),
                  "per_kernel_ms_per_step": prof})

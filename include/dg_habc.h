@@ -36,6 +36,17 @@ extern "C" {
 
 typedef struct dg_solver dg_solver; /* opaque, owned by the library; free with dg_destroy */
 
+/* dg_options.kernel: which kernel runs the fused 3D volume + surface + update stage (eq (41)-(43)).
+ * All of them compute the same stage; they differ in how the D_r/D_s/D_t and LIFT contractions are carried out. */
+#define DG_KERNEL_AUTO 0   /* fp64: MMA for N <= 4, WS at N = 5, TPG for N >= 6; fp32: SCALAR for N <= 2, TF32 for
+                              N = 3..5, TPG for N >= 6 */
+#define DG_KERNEL_SCALAR 1 /* scalar FMA, operators in shared memory (or L1/L2 for high N); fp64 and fp32, N = 1..8 */
+#define DG_KERNEL_MMA 2    /* fp64 DMMA (mma.sync.m8n8k4.f64), operator rows register-resident; N = 1..5 */
+#define DG_KERNEL_WS 3     /* DG_KERNEL_MMA with warp-specialised loader / operand / MMA roles; fp64, N = 4, 5 */
+#define DG_KERNEL_TF32 4   /* fp32 on the tensor cores as error-compensated 3xTF32 (fp32-accurate); N = 3..5 */
+#define DG_KERNEL_TPG 5    /* tensor-pipe kernels for the degrees whose operators do not fit the register file:
+                              fp64 DMMA / fp32 3xTF32; N = 6..8 */
+
 /* Tetrahedral mesh of a cuboid.  Any vertex order inside a tetrahedron is accepted
  * (negatively oriented cells are re-oriented internally).  The six planes bounding the vertex cloud are the
  * domain faces; each carries the HABC unless dg_options.face_bc says otherwise. */
@@ -56,13 +67,8 @@ typedef struct {
     uint64_t workspace_bytes; /* size of workspace_dev; see dg_workspace_bytes */
     int32_t use_graph;        /* 1: replay the 5-stage step as a CUDA graph; ignored (plain launches) when stream is NULL,
                                  because the legacy default stream cannot be captured */
-    int32_t kernel;           /* 3D kernel: 0 = the library's choice; 1 = scalar-FMA kernel (any N, fp64/fp32);
-                                 2 = fp64 tensor-pipe (DMMA) kernel, N <= 5; 3 = its warp-specialised form, N = 4, 5
-                                 (the choice at N = 5); 4 = experimental variant of 3 with the update in helper
-                                 warps; 6 = experimental variant of 3 with a software-pipelined MMA loop;
-                                 5 = fp32 tensor-core kernel (3xTF32, fp32-accurate), N = 3..5 (the choice there);
-                                 7 = tensor-pipe kernels with the operators read through L1/L2, N = 6..8 (fp64 DMMA /
-                                 fp32 3xTF32; the choice there); 8 = register-blocked scalar kernel, N = 6..8.  A kernel that does not cover (N, precision) gives DG_EINVAL */
+    int32_t kernel;           /* 3D kernel (one of DG_KERNEL_*): 0 = the library's choice for (precision, N).  A kernel
+                                 that does not cover (N, precision) gives DG_EINVAL */
     int32_t face_bc[6];       /* boundary condition of the six domain faces, index axis * 2 + (1 for the face at the upper
                                  end of the axis): 0 = HABC (the default), 1 = p = 0 (free surface),
                                  2 = rigid wall (n.u = 0).  Auxiliary fields exist only on HABC faces, on the edges
@@ -78,6 +84,8 @@ typedef struct {
     int32_t launches_per_step; /* kernels launched by one time step (5 LSRK stages) */
     double dt;
     uint64_t device_bytes;     /* device memory held by the solver */
+    int32_t kernel;            /* the 3D kernel in use (DG_KERNEL_*, never DG_KERNEL_AUTO) */
+    char kernel_name[44];      /* its name as a profiler lists it, e.g. "k_vol3d_ws<5>" */
 } dg_info;
 
 /* Device bytes dg_create needs for this problem (lets the caller allocate the workspace, e.g. with torch). */

@@ -30,7 +30,8 @@ class _Options(C.Structure):
 class _Info(C.Structure):
     _fields_ = [("N", C.c_int32), ("J", C.c_int32), ("K", C.c_int32), ("Np", C.c_int32), ("Nfp", C.c_int32),
                 ("T", C.c_int32), ("E", C.c_int32), ("C", C.c_int32), ("precision", C.c_int32),
-                ("launches_per_step", C.c_int32), ("dt", C.c_double), ("device_bytes", C.c_uint64)]
+                ("launches_per_step", C.c_int32), ("dt", C.c_double), ("device_bytes", C.c_uint64),
+                ("kernel", C.c_int32), ("kernel_name", C.c_char * 44)]
 
 
 EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_set_source", "dg_step",
@@ -86,6 +87,8 @@ def dg_reference_element(dim: int, N: int):
 
 
 _BC_CODES = {"habc": 0, "dirichlet": 1, "rigid": 2}
+# dg_options.kernel (DG_KERNEL_* of include/dg_habc.h)
+KERNEL_AUTO, KERNEL_SCALAR, KERNEL_MMA, KERNEL_WS, KERNEL_TF32, KERNEL_TPG = range(6)
 
 
 def _face_bc_codes(face_bc):
@@ -138,7 +141,7 @@ class Solver:
         _check(L.dg_create(C.byref(m), N, J, _dp(c), _dp(rho), C.byref(opt), C.byref(self._h)))
         info = _Info()
         _check(L.dg_get_info(self._h, C.byref(info)))
-        self.info = {k: getattr(info, k) for k, _ in _Info._fields_}
+        self.info = self._info_dict(info)
         for k, v in self.info.items():
             setattr(self, k, v)
 
@@ -159,10 +162,16 @@ class Solver:
         _check(L.dg_set_source(self._h, _dp(xyz), float(f_peak), float(t_s), float(amplitude)))
         self.launches_per_step = self.info["launches_per_step"] = self._refresh_info()["launches_per_step"]
 
+    @staticmethod
+    def _info_dict(info):
+        d = {k: getattr(info, k) for k, _ in _Info._fields_}
+        d["kernel_name"] = d["kernel_name"].decode()
+        return d
+
     def _refresh_info(self):
         info = _Info()
         _check(lib().dg_get_info(self._h, C.byref(info)))
-        return {k: getattr(info, k) for k, _ in _Info._fields_}
+        return self._info_dict(info)
 
     def step(self, nsteps: int = 1):
         _check(lib().dg_step(self._h, int(nsteps)))
@@ -201,6 +210,7 @@ class Solver:
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
+            self._stream.synchronize()          # dg_step is asynchronous: finish before the workspace goes back to torch
             lib().dg_destroy(self._h)
             self._h = C.c_void_p()
             self._ws = None

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdg_habc.so")
 SOURCES = ["dg_api.cu", "mesh.cpp", "refelem.cpp"]
-HEADERS = ["kernels.cuh", "kernels_aux.cuh", "kernel_vol3d_mma.cuh", "kernel_vol3d_ws.cuh", "kernel_vol3d_ws2.cuh", "kernel_vol3d_wsp.cuh", "kernel_vol3d_tf32.cuh", "kernel_vol3d_mmag.cuh", "kernel_vol3d_tf32g.cuh", "mesh.hpp", "refelem.hpp", "habc_coef.hpp",
+HEADERS = ["kernels.cuh", "kernels_aux.cuh", "kernel_vol3d_mma.cuh", "kernel_vol3d_ws.cuh", "kernel_vol3d_tf32.cuh", "kernel_vol3d_mmag.cuh", "kernel_vol3d_tf32g.cuh", "mesh.hpp", "refelem.hpp", "habc_coef.hpp",
            os.path.join("..", "..", "include", "dg_habc.h")]
 
 
@@ -35,7 +35,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc(), "-O3", "-std=c++17", "-shared", "-Xcompiler", "-fPIC",
            "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
            "-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
-    cmd[1:1] = os.environ.get("DG_NVCC_EXTRA", "").split()      # e.g. -DWS2_HV=3 for kernel tuning experiments
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))

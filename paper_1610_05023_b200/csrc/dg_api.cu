@@ -3,6 +3,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstring>
 #include <map>
 #include <set>
@@ -17,8 +18,6 @@
 #include "kernels_aux.cuh"
 #include "kernel_vol3d_mma.cuh"
 #include "kernel_vol3d_ws.cuh"
-#include "kernel_vol3d_ws2.cuh"
-#include "kernel_vol3d_wsp.cuh"
 #include "kernel_vol3d_tf32.cuh"
 #include "kernel_vol3d_mmag.cuh"
 #include "kernel_vol3d_tf32g.cuh"
@@ -81,15 +80,8 @@ struct dg_solver {
     int grid3 = 0;
     int face_grid = 148 * 8;        // persistent CTAs of the 2D solver kernel (set from the SM count in dg_create)
     size_t smem3 = 0;
-    int kernel = 0;                 // dg_options.kernel as requested
-    bool mma3 = false;              // the tensor-pipe 3D kernel is in use
-    bool ws3 = false;               // ... in its warp-specialised form (kernel_vol3d_ws.cuh)
-    bool tfg = false;               // fp32, N >= 6: 3xTF32 tensor-core kernel with the operators read through L1/L2
-    bool mmag = false;              // fp64, N >= 6: tensor-pipe kernel with the operators read through L1/L2 (kernel_vol3d_mmag.cuh)
-    bool ws6 = false;               // ... with the software-pipelined MMA loop (kernel_vol3d_wsp.cuh); implies ws3
-    bool ws4 = false;               // ... with the update in its own warpgroup (kernel_vol3d_ws2.cuh); implies ws3
+    int kern3 = 0;                  // the 3D kernel in use (enum Kern3, resolved from dg_options.kernel in dg_create)
     const void* geox3 = nullptr;    // [Kp][GX3] per-tet record of the warp-specialised kernels (dt folded in), fp64 or fp32
-    bool tf3 = false;               // fp32: the 3xTF32 tensor-core 3D kernel is in use (kernel_vol3d_tf32.cuh)
     bool use_graph = true;
     cudaGraphExec_t graph[2] = {nullptr, nullptr};
     std::vector<double> rho, c;
@@ -98,7 +90,9 @@ struct dg_solver {
     int src_k = 0;
     double src_f = 0, src_ts = 0, src_amp = 0;
     void* src_w = nullptr;          // [Np] of T
-    double* t_dev = nullptr;        // simulated time at the start of the current step
+    double* t_dev = nullptr;        // simulated time at the start of the current step (advanced by k_source while a source is on)
+    double t_host = 0;              // the same clock kept on the host (dg_step adds dt per step), so that a source
+                                    // switched on after some steps starts at the right time
     double* export_buf = nullptr;   // device scratch for dg_get_fields (aux fields, fp64)
     size_t export_elems = 0;
 };
@@ -106,6 +100,32 @@ struct dg_solver {
 namespace {
 
 using namespace dg;
+
+// The 3D kernels.  The values are dg_options.kernel (include/dg_habc.h); KERNELS says what each one covers and
+// DEFAULT_KERNEL which one runs when the caller asks for 0.
+enum Kern3 : int { K3_AUTO = 0, K3_SCALAR = 1, K3_MMA = 2, K3_WS = 3, K3_TF32 = 4, K3_TPG = 5, K3_COUNT };
+
+struct KernRow { int precision /* 0: both */, nmin, nmax; bool geox /* reads the extended per-tet record */; const char* what; };
+const KernRow KERNELS[K3_COUNT] = {
+    {0, 1, 8, false, "auto"},
+    {0, 1, 8, false, "scalar-FMA kernel (kernel = 1): fp64/fp32, N = 1..8"},
+    {64, 1, 5, false, "fp64 tensor-pipe kernel (kernel = 2): fp64, N = 1..5"},
+    {64, 4, 5, true, "warp-specialised fp64 tensor-pipe kernel (kernel = 3): fp64, N = 4, 5"},
+    {32, 3, 5, true, "fp32 3xTF32 tensor-core kernel (kernel = 4): fp32, N = 3..5"},
+    {0, 6, 8, false, "tensor-pipe kernels with operators read through L1/L2 (kernel = 5): N = 6..8"},
+};
+//                                    N =      1          2          3        4        5      6       7       8
+const int DEFAULT_KERNEL_F64[9] = {0, K3_MMA,    K3_MMA,    K3_MMA,  K3_MMA,  K3_WS,   K3_TPG, K3_TPG, K3_TPG};
+const int DEFAULT_KERNEL_F32[9] = {0, K3_SCALAR, K3_SCALAR, K3_TF32, K3_TF32, K3_TF32, K3_TPG, K3_TPG, K3_TPG};
+
+int resolve_kernel(int requested, int precision, int N) {
+    if (requested < 0 || requested >= K3_COUNT) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..5");
+    const int k = requested != K3_AUTO ? requested : (precision == 64 ? DEFAULT_KERNEL_F64 : DEFAULT_KERNEL_F32)[N];
+    const KernRow& r = KERNELS[k];
+    if ((r.precision && r.precision != precision) || N < r.nmin || N > r.nmax)
+        throw std::runtime_error(std::string("EINVAL: the ") + r.what + " does not cover this (precision, N)");
+    return k;
+}
 
 // ---------------------------------------------------------------- device image of the problem
 template <typename T>
@@ -193,7 +213,7 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
         fm3.assign(m.r3.Fmask.begin(), m.r3.Fmask.end());
     }
     d.geo3 = U.real(geo, Kp * GEO3);
-    if (s->ws3 || s->tf3) {
+    if (KERNELS[s->kern3].geox) {
         // record of kernel_vol3d_ws.cuh: G | dt rho c^2, dt/rho, dt c | (Fs n, A)_f | B_f | Fs_f
         std::vector<double> gx;
         if (!A.dry) {
@@ -331,276 +351,111 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
 }
 
 // ---------------------------------------------------------------- kernel dispatch
+// Sizing (configure = true: shared-memory attribute, persistent grid) or launch of one 3D kernel instantiation.
+// per_sm_max = 1 for the kernels that own an SM's register file, else what the occupancy calculator allows.
+template <typename Kern, typename... Args>
+void run_vol3d(dg_solver* s, Kern kern, int nthreads, size_t smem, int elems_per_batch, int K, bool one_per_sm,
+               bool configure, Args... args) {
+    if (configure) {
+        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "smem attr");
+        int per_sm = 1, sms = 0;
+        if (!one_per_sm) cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, nthreads, smem), "occupancy");
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: the 3D kernel does not fit on an SM");
+        const int nbatch = (K + elems_per_batch - 1) / elems_per_batch;
+        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
+        s->smem3 = smem;
+        return;
+    }
+    kern<<<s->grid3, nthreads, smem, s->stream>>>(args...);
+}
+
 template <typename T, int N, int G, int ET, bool SM>
-void launch_vol3d_cfg(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
+void vol3d_scalar(dg_solver* s, Dev<T>& d, int src, double a, double b, bool cfg) {
     using Cfg = Vol3dCfg<T, N, G, ET, SM>;
-    auto kern = k_vol3d<T, N, G, ET, SM>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int per_sm = 0, sms = 0;
-        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        if (per_sm < 1) throw std::runtime_error("ECUDA: volume kernel does not fit on an SM");
-        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
-        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
+    run_vol3d(s, k_vol3d<T, N, G, ET, SM>, Cfg::NT, Cfg::smem_bytes, Cfg::EPB, d.K, false, cfg, d, src, (T)a, (T)b, (T)s->dt);
 }
-
-template <typename T, int N, int NB, int ET, int G>
-void launch_vol3d_rb_cfg(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
-    using Cfg = Vol3dRbCfg<T, N, NB, ET, G>;
-    auto kern = k_vol3d_rb<T, N, NB, ET, G>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int per_sm = 0, sms = 0;
-        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        if (per_sm < 1) throw std::runtime_error("ECUDA: register-blocked volume kernel does not fit on an SM");
-        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
-        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (T)a, (T)b, (T)s->dt);
-}
-
-#ifndef MMAG_NTILE
-#define MMAG_NTILE 2
-#endif
-#ifndef MMAG_W6
-#define MMAG_W6 8
-#endif
-#ifndef MMAG_W7
-#define MMAG_W7 8
-#endif
-#ifndef MMAG_W8
-#define MMAG_W8 8
-#endif
 template <int N>
-void launch_vol3d_mmag_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
-    constexpr int MMAG_W = N == 6 ? MMAG_W6 : N == 7 ? MMAG_W7 : MMAG_W8;
-    using Cfg = MmagCfg<N, MMAG_NTILE, MMAG_W>;
-    auto kern = k_vol3d_mmag<N, MMAG_NTILE, MMAG_W>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int per_sm = 0, sms = 0;
-        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        if (per_sm < 1) throw std::runtime_error("ECUDA: tensor-pipe volume kernel (N >= 6) does not fit on an SM");
-        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
-        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, a, b, s->dt);
+void vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b, bool cfg) {
+    using Cfg = MmaCfg<N>;
+    run_vol3d(s, k_vol3d_mma<N>, Cfg::NT, Cfg::smem_bytes, Cfg::EB, d.K, false, cfg, d, src, a, b, s->dt);
 }
-
 template <int N>
-void launch_vol3d_tf32g_cfg(dg_solver* s, Dev<float>& d, int src, double a, double b, bool configure) {
-    constexpr int TFG_W = N == 6 ? 7 : N == 7 ? 8 : 11;     // warps per CTA, from the sweep in profiles/r02_degree_sweep.md
-    using Cfg = TfgCfg<N, TFG_W>;
-    auto kern = k_vol3d_tf32g<N, TFG_W>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int per_sm = 0, sms = 0;
-        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        if (per_sm < 1) throw std::runtime_error("ECUDA: fp32 tensor-core volume kernel (N >= 6) does not fit on an SM");
-        const int nbatch = (d.K + Cfg::EPB - 1) / Cfg::EPB;
-        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (float)a, (float)b, (float)s->dt);
+void vol3d_ws(dg_solver* s, Dev<double>& d, int src, double a, double b, bool cfg) {
+    using Cfg = WsCfg<N>;
+    run_vol3d(s, k_vol3d_ws<N>, Cfg::NT, Cfg::smem_bytes, Cfg::EB, d.K, true, cfg, d, (const double*)s->geox3, src, a, b);
+}
+template <int N>
+void vol3d_tf32(dg_solver* s, Dev<float>& d, int src, double a, double b, bool cfg) {
+    using Cfg = TfCfg<N>;
+    run_vol3d(s, k_vol3d_tf32<N>, Cfg::NT, Cfg::smem_bytes, Cfg::EB, d.K, true, cfg, d, (const float*)s->geox3, src, (float)a, (float)b);
+}
+template <int N>
+void vol3d_mmag(dg_solver* s, Dev<double>& d, int src, double a, double b, bool cfg) {
+    using Cfg = MmagCfg<N, 2, 8>;                            // 2 n-tiles (16 elements) per batch, 8 warps
+    run_vol3d(s, k_vol3d_mmag<N, 2, 8>, Cfg::NT, Cfg::smem_bytes, Cfg::EPB, d.K, false, cfg, d, src, a, b, s->dt);
+}
+template <int N>
+void vol3d_tf32g(dg_solver* s, Dev<float>& d, int src, double a, double b, bool cfg) {
+    constexpr int W = N == 6 ? 7 : N == 7 ? 8 : 11;          // warps per CTA, from the sweep in profiles/r02_degree_sweep.md
+    using Cfg = TfgCfg<N, W>;
+    run_vol3d(s, k_vol3d_tf32g<N, W>, Cfg::NT, Cfg::smem_bytes, Cfg::EPB, d.K, false, cfg, d, src, (float)a, (float)b, (float)s->dt);
 }
 
-// register blocking of k_vol3d_rb, from the sweep in profiles/r02_degree_sweep.md (fp64: 3 elements per warp, fp32: 4)
-template <typename T> struct RbEt { static constexpr int value = 3; };
-template <> struct RbEt<float> { static constexpr int value = 4; };
-
-template <typename T> struct OpsFit;
+template <typename T> struct OpsFit;                         // scalar kernel: degrees whose operators fit shared memory
 template <> struct OpsFit<double> { static constexpr int maxN = 5; };
 template <> struct OpsFit<float> { static constexpr int maxN = 6; };
 
-// fp64 tensor-pipe kernel (kernel_vol3d_mma.cuh): degrees whose A fragments fit the register file
-constexpr int MMA_MAX_N = 5;
-
-template <int N>
-void launch_vol3d_mma_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
-    using Cfg = MmaCfg<N>;
-    auto kern = k_vol3d_mma<N>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int per_sm = 0, sms = 0;
-        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::NT, Cfg::smem_bytes), "occupancy");
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        if (per_sm < 1) throw std::runtime_error("ECUDA: tensor-pipe volume kernel does not fit on an SM");
-        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
-        s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, a, b, s->dt);
-}
-
-template <int N>
-void launch_vol3d_ws_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
-    using Cfg = WsCfg<N>;
-    auto kern = k_vol3d_ws<N>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int sms = 0;
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
-        s->grid3 = std::max(1, std::min(nbatch, sms));       // one persistent CTA per SM (it owns the register file)
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const double*)s->geox3, src, a, b);
-}
-
-template <int N>
-void launch_vol3d_ws2_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
-    using Cfg = Ws2Cfg<N>;
-    auto kern = k_vol3d_ws2<N>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int sms = 0;
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
-        s->grid3 = std::max(1, std::min(nbatch, sms));       // one persistent CTA per SM (it owns the register file)
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const double*)s->geox3, src, a, b);
-}
-
-template <int N>
-void launch_vol3d_wsp_cfg(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
-    using Cfg = WspCfg<N>;
-    auto kern = k_vol3d_wsp<N>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int sms = 0;
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
-        s->grid3 = std::max(1, std::min(nbatch, sms));       // one persistent CTA per SM (it owns the register file)
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const double*)s->geox3, src, a, b);
-}
-
-void launch_vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
-    if (s->ws6) {
-        switch (s->N) {
-            case 4: return launch_vol3d_wsp_cfg<4>(s, d, src, a, b, configure);
-            case 5: return launch_vol3d_wsp_cfg<5>(s, d, src, a, b, configure);
-            default: throw std::runtime_error("EINVAL: the warp-specialised kernels cover N = 4, 5");
-        }
-    }
-    if (s->ws4) {
-        switch (s->N) {
-            case 4: return launch_vol3d_ws2_cfg<4>(s, d, src, a, b, configure);
-            case 5: return launch_vol3d_ws2_cfg<5>(s, d, src, a, b, configure);
-            default: throw std::runtime_error("EINVAL: the warp-specialised kernels cover N = 4, 5");
-        }
-    }
-    if (s->ws3) {
-        switch (s->N) {
-            case 4: return launch_vol3d_ws_cfg<4>(s, d, src, a, b, configure);
-            case 5: return launch_vol3d_ws_cfg<5>(s, d, src, a, b, configure);
-            default: throw std::runtime_error("EINVAL: the warp-specialised kernel covers N = 4, 5");
-        }
-    }
-    switch (s->N) {
-        case 1: launch_vol3d_mma_cfg<1>(s, d, src, a, b, configure); break;
-        case 2: launch_vol3d_mma_cfg<2>(s, d, src, a, b, configure); break;
-        case 3: launch_vol3d_mma_cfg<3>(s, d, src, a, b, configure); break;
-        case 4: launch_vol3d_mma_cfg<4>(s, d, src, a, b, configure); break;
-        case 5: launch_vol3d_mma_cfg<5>(s, d, src, a, b, configure); break;
-        default: throw std::runtime_error("EINVAL: the tensor-pipe kernel covers N = 1..5");
-    }
-}
-
-template <int N>
-void launch_vol3d_tf32_cfg(dg_solver* s, Dev<float>& d, int src, double a, double b, bool configure) {
-    using Cfg = TfCfg<N>;
-    auto kern = k_vol3d_tf32<N>;
-    if (configure) {
-        cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
-        int sms = 0;
-        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        const int nbatch = (d.K + Cfg::EB - 1) / Cfg::EB;
-        s->grid3 = std::max(1, std::min(nbatch, sms));       // one persistent CTA per SM (it owns the register file)
-        s->smem3 = Cfg::smem_bytes;
-        return;
-    }
-    kern<<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, (const float*)s->geox3, src, (float)a, (float)b);
-}
-
-constexpr int TF32_MIN_N = 3, TF32_MAX_N = 5;
-
-void launch_vol3d_tf32(dg_solver* s, Dev<float>& d, int src, double a, double b, bool configure) {
-    switch (s->N) {
-        case 3: return launch_vol3d_tf32_cfg<3>(s, d, src, a, b, configure);
-        case 4: return launch_vol3d_tf32_cfg<4>(s, d, src, a, b, configure);
-        case 5: return launch_vol3d_tf32_cfg<5>(s, d, src, a, b, configure);
-        default: throw std::runtime_error("EINVAL: the fp32 tensor-core kernel covers N = 3..5");
-    }
-}
-
+#define DG_CASE(n, call) case n: return call
 template <typename T>
-void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure) {
+void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool cfg) {
+    constexpr bool F64 = std::is_same<T, double>::value;
     constexpr int mx = OpsFit<T>::maxN;
-    if constexpr (std::is_same<T, double>::value) {
-        if (s->mmag) {
-            switch (s->N) {
-                case 6: return launch_vol3d_mmag_cfg<6>(s, d, src, a, b, configure);
-                case 7: return launch_vol3d_mmag_cfg<7>(s, d, src, a, b, configure);
-                case 8: return launch_vol3d_mmag_cfg<8>(s, d, src, a, b, configure);
-                default: break;
+    const int N = s->N;
+    switch (s->kern3) {
+        case K3_SCALAR:
+            switch (N) {
+                DG_CASE(1, (vol3d_scalar<T, 1, 32, 4, true>(s, d, src, a, b, cfg)));
+                DG_CASE(2, (vol3d_scalar<T, 2, 16, 4, true>(s, d, src, a, b, cfg)));
+                DG_CASE(3, (vol3d_scalar<T, 3, 8, 4, true>(s, d, src, a, b, cfg)));
+                DG_CASE(4, (vol3d_scalar<T, 4, 8, 4, true>(s, d, src, a, b, cfg)));
+                DG_CASE(5, (vol3d_scalar<T, 5, 4, 4, true>(s, d, src, a, b, cfg)));
+                DG_CASE(6, (vol3d_scalar<T, 6, 4, 2, (6 <= mx)>(s, d, src, a, b, cfg)));
+                DG_CASE(7, (vol3d_scalar<T, 7, 2, 4, false>(s, d, src, a, b, cfg)));
+                DG_CASE(8, (vol3d_scalar<T, 8, 2, 2, false>(s, d, src, a, b, cfg)));
             }
-        }
-    }
-    if constexpr (std::is_same<T, float>::value) {
-        if (s->tf3) return launch_vol3d_tf32(s, d, src, a, b, configure);
-        if (s->tfg) {
-            switch (s->N) {
-                case 6: return launch_vol3d_tf32g_cfg<6>(s, d, src, a, b, configure);
-                case 7: return launch_vol3d_tf32g_cfg<7>(s, d, src, a, b, configure);
-                case 8: return launch_vol3d_tf32g_cfg<8>(s, d, src, a, b, configure);
-                default: break;
+            break;
+        case K3_MMA:
+            if constexpr (F64) switch (N) {
+                DG_CASE(1, vol3d_mma<1>(s, d, src, a, b, cfg)); DG_CASE(2, vol3d_mma<2>(s, d, src, a, b, cfg));
+                DG_CASE(3, vol3d_mma<3>(s, d, src, a, b, cfg)); DG_CASE(4, vol3d_mma<4>(s, d, src, a, b, cfg));
+                DG_CASE(5, vol3d_mma<5>(s, d, src, a, b, cfg));
             }
-        }
-    }
-    if constexpr (std::is_same<T, double>::value) {
-        if (s->mma3) return launch_vol3d_mma(s, d, src, a, b, configure);
-    }
-    switch (s->N) {
-        case 1: launch_vol3d_cfg<T, 1, 32, 4, true>(s, d, src, a, b, configure); break;
-        case 2: launch_vol3d_cfg<T, 2, 16, 4, true>(s, d, src, a, b, configure); break;
-        case 3: launch_vol3d_cfg<T, 3, 8, 4, true>(s, d, src, a, b, configure); break;
-        case 4: launch_vol3d_cfg<T, 4, 8, 4, true>(s, d, src, a, b, configure); break;
-        case 5: launch_vol3d_cfg<T, 5, 4, 4, true>(s, d, src, a, b, configure); break;
-        case 6:
-            if (s->kernel == 1) launch_vol3d_cfg<T, 6, 4, 2, (6 <= mx)>(s, d, src, a, b, configure);
-            else launch_vol3d_rb_cfg<T, 6, 3, RbEt<T>::value, 4>(s, d, src, a, b, configure);
             break;
-        case 7:
-            if (s->kernel == 1) launch_vol3d_cfg<T, 7, 2, 4, false>(s, d, src, a, b, configure);
-            else launch_vol3d_rb_cfg<T, 7, 4, RbEt<T>::value, 4>(s, d, src, a, b, configure);
+        case K3_WS:
+            if constexpr (F64) switch (N) {
+                DG_CASE(4, vol3d_ws<4>(s, d, src, a, b, cfg)); DG_CASE(5, vol3d_ws<5>(s, d, src, a, b, cfg));
+            }
             break;
-        case 8:
-            if (s->kernel == 1) launch_vol3d_cfg<T, 8, 2, 2, false>(s, d, src, a, b, configure);
-            else launch_vol3d_rb_cfg<T, 8, 6, 2, 4>(s, d, src, a, b, configure);
+        case K3_TF32:
+            if constexpr (!F64) switch (N) {
+                DG_CASE(3, vol3d_tf32<3>(s, d, src, a, b, cfg)); DG_CASE(4, vol3d_tf32<4>(s, d, src, a, b, cfg));
+                DG_CASE(5, vol3d_tf32<5>(s, d, src, a, b, cfg));
+            }
             break;
-        default: throw std::runtime_error("EINVAL: N must be in 1..8");
+        case K3_TPG:
+            if constexpr (F64) switch (N) {
+                DG_CASE(6, vol3d_mmag<6>(s, d, src, a, b, cfg)); DG_CASE(7, vol3d_mmag<7>(s, d, src, a, b, cfg));
+                DG_CASE(8, vol3d_mmag<8>(s, d, src, a, b, cfg));
+            } else switch (N) {
+                DG_CASE(6, vol3d_tf32g<6>(s, d, src, a, b, cfg)); DG_CASE(7, vol3d_tf32g<7>(s, d, src, a, b, cfg));
+                DG_CASE(8, vol3d_tf32g<8>(s, d, src, a, b, cfg));
+            }
+            break;
     }
+    throw std::runtime_error("EINVAL: no 3D kernel for this (kernel, precision, N)");     // resolve_kernel rules this out
 }
+#undef DG_CASE
 
 template <typename T>
 void launch_face2d(dg_solver* s, Dev<T>& d, int src, double a, double b) {
@@ -679,13 +534,23 @@ void run_steps(dg_solver* s, Dev<T>& d, int nsteps) {
     for (int i = 0; i < nsteps; ++i) {
         const int par = s->cur;
         if (!s->graph[par]) {
-            cudaGraph_t g;
+            cudaGraph_t g = nullptr;
             cu(cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal), "begin capture");
-            run_step_plain<T>(s, d);
+            try {
+                run_step_plain<T>(s, d);
+                cu(cudaGetLastError(), "kernel launch (capture)");
+            } catch (...) {                // never leave the caller's stream in capture mode
+                cudaStreamEndCapture(s->stream, &g);
+                if (g) cudaGraphDestroy(g);
+                cudaGetLastError();
+                s->cur = par;
+                throw;
+            }
             cu(cudaStreamEndCapture(s->stream, &g), "end capture");
-            cu(cudaGraphInstantiate(&s->graph[par], g, 0), "graph instantiate");
+            const cudaError_t e = cudaGraphInstantiate(&s->graph[par], g, 0);
             cudaGraphDestroy(g);
             s->cur = par;              // capture did not execute anything
+            cu(e, "graph instantiate");
         }
         cu(cudaGraphLaunch(s->graph[par], s->stream), "graph launch");
         s->cur = par ^ 1;              // five stages flip the parity once
@@ -729,6 +594,7 @@ void upload_initial(dg_solver* s, Dev<T>& d, const double* p, const double* u, c
     if (n2) cu(cudaMemsetAsync(d.fres, 0, sizeof(T) * n2, s->stream), "memset");
     if (n1) cu(cudaMemsetAsync(d.eres, 0, sizeof(T) * n1, s->stream), "memset");
     s->cur = 0;
+    s->t_host = 0;
     cu(cudaMemsetAsync(s->t_dev, 0, sizeof(double), s->stream), "memset");
     launch_closures<T>(s, d, 0);        // reading R5: cached r^-, S consistent with the initial state
     cu(cudaStreamSynchronize(s->stream), "set_initial");
@@ -869,8 +735,9 @@ int dg_workspace_bytes(const dg_mesh* mesh, int N, int J, int precision, uint64_
         if (!bytes) throw std::runtime_error("EINVAL: NULL argument");
         dg_solver s;
         s.N = N; s.J = J; s.precision = precision;
-        s.ws3 = precision == 64 && N >= 4 && N <= 5;           // upper bound: covers every dg_options.kernel choice
-        s.tf3 = precision == 32 && N >= TF32_MIN_N && N <= TF32_MAX_N;
+        s.kern3 = K3_SCALAR;                                   // upper bound over every dg_options.kernel choice:
+        for (int k = 1; k < K3_COUNT; ++k)                     // a kernel with the extended per-tet record, if one covers (precision, N)
+            if (KERNELS[k].geox && (!KERNELS[k].precision || KERNELS[k].precision == precision) && N >= KERNELS[k].nmin && N <= KERNELS[k].nmax) s.kern3 = k;
         s.m.N = N; s.m.K = mesh->ntets; s.m.C = 8;
         quick_counts(mesh, s.m.T, s.m.E);
         s.m.Np = (N + 1) * (N + 2) * (N + 3) / 6; s.m.Nfp = (N + 1) * (N + 2) / 2; s.m.N1 = N + 1;
@@ -893,24 +760,8 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->device = opt ? opt->device : 0;
         s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
         s->use_graph = opt ? opt->use_graph != 0 : true;
-        s->kernel = opt ? opt->kernel : 0;
-        if (s->kernel < 0 || s->kernel > 8) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..8");
-        if (s->kernel == 8 && N < 6) throw std::runtime_error("EINVAL: kernel = 8 covers N = 6..8");
-        if (s->kernel == 7 && N < 6) throw std::runtime_error("EINVAL: kernel = 7 covers N = 6..8");
-        if (s->kernel == 5 && (precision != 32 || N < TF32_MIN_N || N > TF32_MAX_N))
-            throw std::runtime_error("EINVAL: the fp32 tensor-core kernel (kernel = 5) covers fp32, N = 3..5");
-        if ((s->kernel == 3 || s->kernel == 4 || s->kernel == 6) && (precision != 64 || N < 4 || N > 5))
-            throw std::runtime_error("EINVAL: the warp-specialised kernels (kernel = 3, 4, 6) cover fp64, N = 4, 5");
-        if (s->kernel == 2 && (precision != 64 || N > MMA_MAX_N))
-            throw std::runtime_error("EINVAL: the tensor-pipe kernel (kernel = 2) covers fp64, N = 1..5");
+        s->kern3 = resolve_kernel(opt ? opt->kernel : 0, precision, N);
         if (mesh->ntets > CONN_MAX_ID) throw std::runtime_error("EINVAL: more than 2^26 - 1 tetrahedra");
-        s->mma3 = precision == 64 && N <= MMA_MAX_N && s->kernel != 1;
-        s->tf3 = precision == 32 && N >= TF32_MIN_N && N <= TF32_MAX_N && (s->kernel == 0 || s->kernel == 5);
-        s->mmag = precision == 64 && N >= 6 && (s->kernel == 0 || s->kernel == 7);
-        s->tfg = precision == 32 && N >= 6 && (s->kernel == 0 || s->kernel == 7);
-        s->ws4 = s->mma3 && s->kernel == 4;
-        s->ws6 = s->mma3 && s->kernel == 6;
-        s->ws3 = s->mma3 && (s->ws4 || s->ws6 || s->kernel == 3 || (s->kernel == 0 && N == 5));
         if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured
         s->rho.assign(rho, rho + mesh->ntets);
         s->c.assign(c, c + mesh->ntets);
@@ -959,6 +810,8 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
 
 void dg_destroy(dg_solver* s) {
     if (!s) return;
+    cudaSetDevice(s->device);
+    cudaStreamSynchronize(s->stream);      // dg_step is asynchronous: nothing may still be writing the workspace
     for (int i = 0; i < 2; ++i) if (s->graph[i]) cudaGraphExecDestroy(s->graph[i]);
     if (s->own_ws && s->ws) cudaFree(s->ws);
     delete s;
@@ -970,6 +823,10 @@ int dg_get_info(const dg_solver* s, dg_info* o) {
     o->T = s->m.T; o->E = s->m.E; o->C = s->m.C; o->precision = s->precision;
     o->launches_per_step = 5 * launches_per_stage(s);
     o->dt = s->dt; o->device_bytes = s->ws_bytes;
+    o->kernel = s->kern3;
+    static const char* const NAMES[K3_COUNT][2] = {{"", ""}, {"k_vol3d", "k_vol3d"}, {"k_vol3d_mma", ""}, {"k_vol3d_ws", ""},
+                                                   {"", "k_vol3d_tf32"}, {"k_vol3d_mmag", "k_vol3d_tf32g"}};
+    snprintf(o->kernel_name, sizeof(o->kernel_name), "%s<%d>", NAMES[s->kern3][s->precision == 32], s->N);
     return DG_OK;
 }
 
@@ -1045,6 +902,8 @@ int dg_set_source(dg_solver* s, const double* xyz, double f_peak, double t_s, do
             std::vector<float> wf(w.begin(), w.end());
             cu(cudaMemcpy(s->src_w, wf.data(), sizeof(float) * wf.size(), cudaMemcpyHostToDevice), "upload weights");
         }
+        // the device clock only runs while a source is on: bring it to the time reached so far
+        cu(cudaMemcpy(s->t_dev, &s->t_host, sizeof(double), cudaMemcpyHostToDevice), "upload clock");
         s->src_k = kfound; s->src_f = f_peak; s->src_ts = t_s; s->src_amp = amplitude;
         s->src_on = amplitude != 0.0;
         for (int i = 0; i < 2; ++i)                 // the captured step no longer matches
@@ -1059,6 +918,7 @@ int dg_step(dg_solver* s, int nsteps) {
         cu(cudaSetDevice(s->device), "cudaSetDevice");
         if (s->precision == 64) run_steps<double>(s, s->d64, nsteps);
         else run_steps<float>(s, s->d32, nsteps);
+        for (int i = 0; i < nsteps; ++i) s->t_host += s->dt;
         return DG_OK;
     } catch (const std::exception& e) { return err_from_exception(e); }
 }

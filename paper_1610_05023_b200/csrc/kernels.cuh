@@ -256,201 +256,4 @@ k_vol3d(Dev<T> d, int src, T rka, T rkb, T dt) {
     }
 }
 
-
-// =====================================================================================================
-// 3D, register-blocked scalar kernel for the degrees whose operators do not fit the register file of the
-// tensor-pipe kernels (N >= 6).  Same fused stage as k_vol3d.  One WARP per group of ET elements; lane `slot`
-// owns the NB nodes slot, slot + SL, slot + 2 SL, ... (SL = ceil(Np / NB) <= 32), so an operator entry fetched
-// from L1/L2 feeds ET elements and a field value broadcast from shared memory feeds NB nodes:
-// (6 NB + 8 ET) L1 wavefronts per 6 NB ET FMA instead of the 1.3 per FMA of k_vol3d, which is what bounds it at
-// 18-27 % of the fp64 roof for N = 6..8 (profiles/r02_degree_sweep.md).
-// =====================================================================================================
-template <typename T, int N, int NB, int ET, int G>
-struct Vol3dRbCfg {
-    static constexpr int Np = Deg<N>::Np, Nfp = Deg<N>::Nfp, Nfn = Deg<N>::Nfn;
-    static constexpr int SL = (Np + NB - 1) / NB;      // node slots = active lanes per warp
-    static constexpr int EPB = G * ET;
-    static constexpr int NT = 32 * G;
-    static constexpr size_t smem_bytes = sizeof(T) * (EPB * Np * 4 + Nfn * EPB) + 16;
-    static_assert(SL <= 32, "one warp per element group");
-};
-
-template <typename T, int N, int NB, int ET, int G>
-__global__ void __launch_bounds__(Vol3dRbCfg<T, N, NB, ET, G>::NT)
-k_vol3d_rb(Dev<T> d, int src, T rka, T rkb, T dt) {
-    using Cfg = Vol3dRbCfg<T, N, NB, ET, G>;
-    constexpr int Np = Cfg::Np, Nfp = Cfg::Nfp, Nfn = Cfg::Nfn, EPB = Cfg::EPB, NT = Cfg::NT, SL = Cfg::SL;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    T* sm = reinterpret_cast<T*>(smem_raw);
-    Q4<T>* sQ = reinterpret_cast<Q4<T>*>(sm);           // [EPB][Np]  (p, U^r, U^s, U^t)
-    T* sG = sm + EPB * Np * 4;                          // [Nfn][EPB] flux jump g per face node
-    const T* __restrict__ sD = d.Dt3;                   // [3][Np(m)][Np(n)]
-    const T* __restrict__ sL = d.Lt3;                   // [Nfn(j)][Np(n)]
-    const Q4<T>* __restrict__ qold = reinterpret_cast<const Q4<T>*>(d.q[src]);
-    Q4<T>* __restrict__ qnew = reinterpret_cast<Q4<T>*>(d.q[src ^ 1]);
-    Q4<T>* __restrict__ res = reinterpret_cast<Q4<T>*>(d.res);
-    const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
-    const bool active = lane < SL;
-    const int nbatch = (d.K + EPB - 1) / EPB;
-
-    for (int batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
-        const int e0 = batch * EPB;
-        const int ne = min(EPB, d.K - e0);
-        // ---- phase 1: (p, contravariant velocity) of every node of the batch -> shared
-        for (int idx = tid; idx < EPB * Np; idx += NT) {
-            const int e = idx / Np;
-            Q4<T> c{0, 0, 0, 0};
-            if (e < ne) {
-                const T* g = d.geo3 + (size_t)(e0 + e) * GEO3;
-                const Q4<T> v = qold[(size_t)e0 * Np + idx];
-                c.p = v.p;
-                c.u = g[0] * v.u + g[1] * v.v + g[2] * v.w;
-                c.v = g[3] * v.u + g[4] * v.v + g[5] * v.w;
-                c.w = g[6] * v.u + g[7] * v.v + g[8] * v.w;
-            }
-            sQ[idx] = c;
-        }
-        __syncthreads();
-        // ---- phase 2: flux jump g at every face node (PAPER.md:L499-512 reduced to one scalar)
-        for (int idx = tid; idx < EPB * Nfn; idx += NT) {
-            const int e = idx / Nfn, fj = idx - e * Nfn;
-            T gval = 0;
-            if (e < ne) {
-                const int f = fj / Nfp, j = fj - f * Nfp;
-                const int k = e0 + e;
-                const T* g = d.geo3 + (size_t)k * GEO3;
-                const Q4<T> m = sQ[e * Np + d.fmask3[fj]];
-                const T unM = (f == 0) ? -m.w : (f == 1) ? -m.v : (f == 2) ? (m.u + m.v + m.w) : -m.u;
-                const int nb = d.nbr3[k * 4 + f];
-                T pP, unP;
-                if (nb >= 0) {
-                    const uint32_t info = (d.finfo3[k] >> (8 * f)) & 0xffu;
-                    const int fp = info & 3, pm = info >> 2;
-                    const int np_ = d.fmask3[fp * Nfp + d.perm3[pm * Nfp + j]];
-                    const Q4<T> x = qold[(size_t)nb * Np + np_];
-                    T nx, ny, nz;
-                    if (f == 0) { nx = -g[6]; ny = -g[7]; nz = -g[8]; }
-                    else if (f == 1) { nx = -g[3]; ny = -g[4]; nz = -g[5]; }
-                    else if (f == 2) { nx = g[0] + g[3] + g[6]; ny = g[1] + g[4] + g[7]; nz = g[2] + g[5] + g[8]; }
-                    else { nx = -g[0]; ny = -g[1]; nz = -g[2]; }
-                    pP = x.p;
-                    unP = nx * x.u + ny * x.v + nz * x.w;
-                } else {
-                    pP = T(2) * d.qb3[(size_t)(-1 - nb) * Nfp + j];     // ghost state: p+ = 2 r^-, u+ = 0
-                    unP = 0;
-                }
-                gval = g[9 + f] * (unP - unM) - g[13 + f] * (pP - m.p);
-            }
-            sG[fj * EPB + e] = gval;
-        }
-        __syncthreads();
-        // ---- phase 3: D_r, D_s, D_t contraction and LIFT, NB nodes x ET elements per lane; update
-        if (active) {
-            T dpr[NB][ET], dps[NB][ET], dpt[NB][ET], dvg[NB][ET];
-#pragma unroll
-            for (int i = 0; i < NB; ++i)
-#pragma unroll
-                for (int e = 0; e < ET; ++e) dpr[i][e] = dps[i][e] = dpt[i][e] = dvg[i][e] = 0;
-            const Q4<T>* q0 = sQ + grp * ET * Np;
-            // padded node slots read the last column (results discarded)
-            int nn[NB];
-#pragma unroll
-            for (int i = 0; i < NB; ++i) nn[i] = min(lane + i * SL, Np - 1);
-#pragma unroll 2
-            for (int m = 0; m < Np; ++m) {
-                Q4<T> c[ET];
-#pragma unroll
-                for (int e = 0; e < ET; ++e) c[e] = q0[e * Np + m];
-#pragma unroll
-                for (int i = 0; i < NB; ++i) {
-                    const T dr = sD[m * Np + nn[i]], ds = sD[Np * Np + m * Np + nn[i]], dtt = sD[2 * Np * Np + m * Np + nn[i]];
-#pragma unroll
-                    for (int e = 0; e < ET; ++e) {
-                        dpr[i][e] += dr * c[e].p;
-                        dps[i][e] += ds * c[e].p;
-                        dpt[i][e] += dtt * c[e].p;
-                        dvg[i][e] += dr * c[e].u;
-                        dvg[i][e] += ds * c[e].v;
-                        dvg[i][e] += dtt * c[e].w;
-                    }
-                }
-            }
-            // fold the material constants in: X_a = -1/rho d_a p, then add c * (LIFT combos); dvg += Fs_f LIFT_f g.
-            // rhs_u = G^T (X_r, X_s, X_t), with the reference normals giving X_r += c (a2 - a3), X_s += c (a2 - a1),
-            // X_t += c (a2 - a0)  (a_f = LIFT_f g)
-            T cc_[ET], fs_[ET][4];
-#pragma unroll
-            for (int e = 0; e < ET; ++e) {
-                const int el = min(grp * ET + e, ne - 1);
-                const T* g = d.geo3 + (size_t)(e0 + el) * GEO3;
-                const T irho = g[22];
-                cc_[e] = g[23];
-#pragma unroll
-                for (int f = 0; f < 4; ++f) fs_[e][f] = g[17 + f];
-#pragma unroll
-                for (int i = 0; i < NB; ++i) { dpr[i][e] *= -irho; dps[i][e] *= -irho; dpt[i][e] *= -irho; }
-            }
-#pragma unroll
-            for (int f = 0; f < 4; ++f) {
-                T af[NB][ET];
-#pragma unroll
-                for (int i = 0; i < NB; ++i)
-#pragma unroll
-                    for (int e = 0; e < ET; ++e) af[i][e] = 0;
-                for (int j = 0; j < Nfp; ++j) {
-                    T gg[ET];
-#pragma unroll
-                    for (int e = 0; e < ET; ++e) gg[e] = sG[(f * Nfp + j) * EPB + grp * ET + e];
-#pragma unroll
-                    for (int i = 0; i < NB; ++i) {
-                        const T l = sL[(f * Nfp + j) * Np + nn[i]];
-#pragma unroll
-                        for (int e = 0; e < ET; ++e) af[i][e] += l * gg[e];
-                    }
-                }
-#pragma unroll
-                for (int i = 0; i < NB; ++i)
-#pragma unroll
-                    for (int e = 0; e < ET; ++e) {
-                        const T ca = cc_[e] * af[i][e];
-                        dvg[i][e] += fs_[e][f] * af[i][e];
-                        if (f == 0) dpt[i][e] -= ca;
-                        else if (f == 1) dps[i][e] -= ca;
-                        else if (f == 3) dpr[i][e] -= ca;
-                        else { dpr[i][e] += ca; dps[i][e] += ca; dpt[i][e] += ca; }
-                    }
-            }
-#pragma unroll
-            for (int e = 0; e < ET; ++e) {
-                const int el = grp * ET + e;
-                if (el < ne) {
-                    const T* g = d.geo3 + (size_t)(e0 + el) * GEO3;
-                    const T rc2 = g[21];
-#pragma unroll
-                    for (int i = 0; i < NB; ++i) {
-                        const int n = lane + i * SL;
-                        if (n < Np) {
-                            const T xr = dpr[i][e], xs = dps[i][e], xt = dpt[i][e];
-                            const T rp = -rc2 * dvg[i][e];
-                            const T ru = g[0] * xr + g[3] * xs + g[6] * xt;
-                            const T rv = g[1] * xr + g[4] * xs + g[7] * xt;
-                            const T rw = g[2] * xr + g[5] * xs + g[8] * xt;
-                            const size_t o = (size_t)(e0 + el) * Np + n;
-                            Q4<T> r = res[o];
-                            Q4<T> v = qold[o];
-                            r.p = rka * r.p + dt * rp;  v.p += rkb * r.p;
-                            r.u = rka * r.u + dt * ru;  v.u += rkb * r.u;
-                            r.v = rka * r.v + dt * rv;  v.v += rkb * r.v;
-                            r.w = rka * r.w + dt * rw;  v.w += rkb * r.w;
-                            res[o] = r;
-                            qnew[o] = v;
-                        }
-                    }
-                }
-            }
-        }
-        __syncthreads();
-    }
-}
-
 }  // namespace dg

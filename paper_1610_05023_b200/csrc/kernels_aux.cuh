@@ -42,9 +42,7 @@ __host__ __device__ inline int face2d_ops_elems(int Nfp, int N1) {          // o
     return ((2 * Nfp * Nfp + 3 * N1 * Nfp + 3) / 4) * 4 + 16;
 }
 
-#ifndef FACE2D_MINB
-#define FACE2D_MINB 4
-#endif
+constexpr int FACE2D_MINB = 4;        // resident CTAs per SM the register budget is set for
 template <typename T>
 __global__ void __launch_bounds__(FACE2D_NT, FACE2D_MINB) k_face2d(Dev<T> d, int src, T rka, T rkb, T dt) {
     extern __shared__ __align__(128) unsigned char smem_raw[];

@@ -67,24 +67,61 @@ def run_library(w, precision=64, nsteps=None, dt=0.0, use_graph=True, kernel=0, 
 
 
 def compare(lib, ora):
-    """Relative L2 error per field group (BASELINE north_star: p, u and all auxiliary fields)."""
+    """Relative L2 error of EVERY field on its own (BASELINE north_star: "p, u and all auxiliary fields"): p; the
+    three velocity components; for each face set i the physical p_i00 and each of the two tangential velocities; for
+    each edge set (i,j) p_ij0 and the tangential velocity.  Each against the oracle norm of that same field over all
+    cells.  Returned: one entry per field ("p", "ux", "uy", "uz", "face_p[i]", "face_v1[i]", "face_v2[i]",
+    "edge_p[i,j]", "edge_w[i,j]") plus the group summaries the tests assert on,
+        "u" / "face" / "edge"      = the WORST member of the group,
+        "norm_u" / "norm_face" / "norm_edge" (pressures) / "norm_face_vel" / "norm_edge_vel" = the SMALLEST oracle norm
+    in the group, so that a tolerance on the summary holds per field and per set, and the non-vacuity floor (pin P16)
+    applies to every set separately."""
     ia, ib, perm = match_cells(lib["x"], ora["x"])
     rows = np.arange(len(ia))[:, None]
     ql = lib["q"][:, ia]
     qo = ora["q"][:, ib][:, rows, perm]
-    out = {"p": rel_l2(ql[0], qo[0]), "u": rel_l2(ql[1:], qo[1:]),
-           "norm_p": float(np.linalg.norm(qo[0])), "norm_u": float(np.linalg.norm(qo[1:]))}
+    out = {"p": rel_l2(ql[0], qo[0]), "norm_p": float(np.linalg.norm(qo[0]))}
+    for d, name in enumerate(("ux", "uy", "uz")):
+        out[name] = rel_l2(ql[1 + d], qo[1 + d])
+    out["u"] = max(out[k] for k in ("ux", "uy", "uz"))
+    out["norm_u"] = min(float(np.linalg.norm(qo[1 + d])) for d in range(3))
     if ora["T"] and ora["fa"].size:
         ia, ib, perm = match_cells(lib["xf"], ora["xf"])
-        rows = np.arange(len(ia))[:, None]
         fl = lib["fa"][ia]                                            # [T,J,3,Nfp]
         fo = np.take_along_axis(ora["fa"][ib], perm[:, None, None, :], axis=3)
-        out["face"] = rel_l2(fl, fo)
-        out["norm_face"] = float(np.linalg.norm(fo))
+        norms = {"p": [], "v": []}
+        for i in range(fo.shape[1]):
+            for comp, name in enumerate(("p", "v1", "v2")):
+                out[f"face_{name}[{i}]"] = rel_l2(fl[:, i, comp], fo[:, i, comp])
+                norms["p" if comp == 0 else "v"].append(float(np.linalg.norm(fo[:, i, comp])))
+        out["face"] = max(v for k, v in out.items() if k.startswith("face_"))
+        out["norm_face"], out["norm_face_vel"] = min(norms["p"]), min(norms["v"])
     if ora["E"] and ora["ea"].size:
         ia, ib, perm = match_cells(lib["xe"], ora["xe"])
-        el = lib["ea"][ia]
+        el = lib["ea"][ia]                                            # [E,J*J,2,N1]
         eo = np.take_along_axis(ora["ea"][ib], perm[:, None, None, :], axis=3)
-        out["edge"] = rel_l2(el, eo)
-        out["norm_edge"] = float(np.linalg.norm(eo))
+        J = int(round(np.sqrt(eo.shape[1])))
+        norms = {"p": [], "w": []}
+        for s_ in range(eo.shape[1]):
+            for comp, name in enumerate(("p", "w")):
+                out[f"edge_{name}[{s_ // J},{s_ % J}]"] = rel_l2(el[:, s_, comp], eo[:, s_, comp])
+                norms[name].append(float(np.linalg.norm(eo[:, s_, comp])))
+        out["edge"] = max(v for k, v in out.items() if k.startswith("edge_"))
+        out["norm_edge"], out["norm_edge_vel"] = min(norms["p"]), min(norms["w"])
     return out
+
+
+def worst(err, n=4):
+    """the n largest per-field errors, for assertion messages"""
+    items = [(k, v) for k, v in err.items() if not k.startswith("norm") and k not in ("u", "face", "edge")]
+    return sorted(items, key=lambda kv: -kv[1])[:n]
+
+
+def check(err, tol, aux=True, floor_face=1e-3, floor_edge=1e-4, floor_vel=1e-6):
+    """tolerance on every field and every auxiliary set; pin P16 per set: each one carries data"""
+    for k in ["p", "u"] + (["face", "edge"] if aux else []):
+        assert err[k] <= tol, (k, err[k], worst(err))
+    assert err["norm_p"] > 0
+    if aux:
+        assert err["norm_face"] > floor_face * err["norm_p"] and err["norm_edge"] > floor_edge * err["norm_p"], err
+        assert err["norm_face_vel"] > floor_vel * err["norm_p"] and err["norm_edge_vel"] > floor_vel * err["norm_p"], err
