@@ -25,9 +25,10 @@ from workloads import CONFIGS, make_workload  # noqa: E402
 
 METRIC = "DG+HABC node-updates/sec"
 UNIT = "node-updates/s"
-# measured on this pool's B200 with paper_1610_05023_b200/csrc/ubench/peaks.cu (profiles/r01_peaks.md)
-FP64_TFLOPS_MEASURED = 34.0
-FP32_TFLOPS_MEASURED = 72.0
+# measured on this pool's B200 with paper_1610_05023_b200/csrc/ubench/peaks.cu (profiles/r01_peaks.md): DFMA 36.98,
+# DMMA 37.19 TFLOP/s (the same fp64 unit; the mixed DMMA+DFMA loop of that probe reaches 33.5), FFMA 71.2
+FP64_TFLOPS_MEASURED = 37.0
+FP32_TFLOPS_MEASURED = 71.2
 HBM_FALLBACK_GBS = 6650.0
 
 
@@ -97,7 +98,7 @@ def oracle_sample(workload: str, precision: int, budget_s: float = 20.0):
     cn = np.repeat(w.c[:, None], x.shape[1], axis=1)
     o.set_initial(np.stack(w.fields(x[..., 0], x[..., 1], x[..., 2], cn, 1.0)))
     o.step(1)
-    steps, t0 = 0, time.perf_counter()
+    steps, t0, cpu0 = 0, time.perf_counter(), time.process_time()
     while True:
         o.step(1)
         steps += 1
@@ -105,9 +106,54 @@ def oracle_sample(workload: str, precision: int, budget_s: float = 20.0):
         if el > budget_s or steps >= 50:
             break
     nodes = o.H.tet.K * o.H.tet.ref.Np
-    cores = len(os.sched_getaffinity(0))
-    desc = f"{workload} rule on a {'x'.join(str(m) for m in w.shape)} hex grid ({o.H.tet.K} tets, N={w.N}, J={w.J}), {steps} steps, fp64 numpy"
-    return nodes * steps / el, desc, cores, el / steps
+    # threads the numpy oracle really kept busy: process CPU time over wall time of the timed loop
+    cpu = time.process_time() - cpu0
+    cores = max(1, int(round(cpu / el)))
+    avail = len(os.sched_getaffinity(0))
+    desc = (f"{workload} rule on a {'x'.join(str(m) for m in w.shape)} hex grid ({o.H.tet.K} tets, N={w.N}, J={w.J}), "
+            f"{steps} steps, fp64 numpy; cores = CPU time / wall time = {cpu / el:.2f} of {avail} available")
+    return nodes * steps / el, desc, cores, el / steps, avail
+
+
+def workload_config(name: str, w) -> dict:
+    """The part of `config` that names the workload; both arms (ours and --impl reference) print the same one."""
+    Np = (w.N + 1) * (w.N + 2) * (w.N + 3) // 6
+    return {"workload": name, "n_hex": w.n, "hex_grid": list(w.shape), "N": w.N, "J": w.J, "K": w.K, "nodes": w.K * Np}
+
+
+def roofline(s, w, prec: int, prof: dict, workload: str) -> dict:
+    """Roofline object of the dominant kernel (the fused 3D stage): algorithmic bytes / flops per launch
+    over the launch time measured with CUDA events on the solver's stream, against the measured peaks."""
+    vol_ms = prof["vol3d"] / 5.0                                  # per launch
+    bytes_launch = algorithmic_bytes_per_element(w.N, prec) * s.K
+    flops_launch = algorithmic_flops_per_element(w.N) * s.K
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
+    alu_peak = FP64_TFLOPS_MEASURED if prec == 64 else FP32_TFLOPS_MEASURED
+    hbm = {"bound": "hbm", "achieved": bytes_launch / (vol_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+           "peak_source": "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"}
+    hbm["frac"] = hbm["achieved"] / hbm["peak"]
+    alu = {"bound": "alu", "achieved": flops_launch / (vol_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+           "peak_source": "profiles/r01_peaks.md (DFMA / DMMA / FFMA microbenchmark on this pool: 37.0 / 37.2 / 71.2)"}
+    alu["frac"] = alu["achieved"] / alu["peak"]
+    t_mem, t_alu = bytes_launch / (hbm_peak * 1e9), flops_launch / (alu_peak * 1e12)
+    roof = dict(hbm if t_mem >= t_alu else alu)
+    roof.update({"kernel": s.info["kernel_name"], "ms_per_launch": vol_ms, "traffic": None, "traffic_source": None,
+                 "roof_ms": 1e3 * max(t_mem, t_alu), "frac_of_slower_roof": max(t_mem, t_alu) / (vol_ms * 1e-3),
+                 "hbm": hbm, "alu": alu, "kernel_share_of_step": prof["vol3d"] / max(sum(prof.values()), 1e-12),
+                 "per_kernel_ms_per_step": prof})
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")     # from the ncu --set full captures under profiles/
+    if os.path.exists(traffic_file):
+        for ln in open(traffic_file).read().splitlines()[1:]:
+            cols = ln.split(",", 3)
+            if len(cols) == 4 and cols[0] == f"{workload}_f{prec}" and cols[2] == s.info["kernel_name"]:
+                roof["traffic"] = float(cols[1])
+                roof["traffic_source"] = f"static: ncu --set full capture of {cols[2]} recorded in profiles/traffic.csv ({cols[3]}); not measured in this run"
+    return roof
 
 
 def run_reference(args):
@@ -117,51 +163,30 @@ def run_reference(args):
     per_step_budget = 6.0
     vals = []
     for _ in range(args.warmup + args.steps):
-        v, desc, cores, step_s = oracle_sample(args.workload, 64, budget_s=per_step_budget)
+        v, desc, cores, step_s, avail = oracle_sample(args.workload, 64, budget_s=per_step_budget)
         vals.append((v, step_s))
     vals = vals[args.warmup:]
     value = float(np.mean([v for v, _ in vals]))
-    d = CONFIGS[args.workload]
+    w = make_workload(args.workload, n=args.n, N=args.N, J=args.J)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([s for _, s in vals])),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "n_hex": d["n"], "N": d["N"], "J": d["J"]},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "config": dict(workload_config(args.workload, w), parallelism="replicas only" if args.gpus > 1 else "single GPU",
+                           l2="state (q,res) exceeds L2 many times over; no flush needed"),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "cores_available": avail, "kind": "oracle",
+                             "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg5")
-    ap.add_argument("--precision", type=int, default=64)
-    ap.add_argument("--n", type=int, default=None, help="override hexes per side (debug only; invalidates the metric)")
-    ap.add_argument("--N", type=int, default=None, help="override the polynomial degree (degree sweep of configs[3])")
-    ap.add_argument("--J", type=int, default=None, help="override the HABC order (degree sweep of configs[3])")
-    ap.add_argument("--impl", default="ours")
-    ap.add_argument("--kernel", type=int, default=0, help="dg_options.kernel (0 = the library's choice)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
-    if args.impl == "reference":
-        return run_reference(args)
-
+def measure(args, w, prec: int, rep, local: int) -> dict:
+    """One precision: set the problem up, time `steps` steps device-resident, the per-kernel times and roofline, and
+    the end-to-end run through the C ABI with host buffers."""
     import torch
     from paper_1610_05023_b200 import Solver
-    from paper_1610_05023_b200.replicas import Replicas
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    rep = Replicas.from_env("nccl")
-    rank, world, local = rep.rank, rep.world, rep.local
-    torch.cuda.set_device(local)
-
-    w = make_workload(args.workload, n=args.n, N=args.N, J=args.J)
-    prec = args.precision
+    world = rep.world
     t_setup = time.perf_counter()
     s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, kernel=args.kernel, face_bc=w.face_bc)
     x, y, z = s.get_nodes()
@@ -171,7 +196,6 @@ def main():
     s.set_initial(*fields)
     t_setup = time.perf_counter() - t_setup
     nodes = s.K * s.Np
-
     barrier = rep.barrier
 
     # ---- device-resident throughput
@@ -195,34 +219,7 @@ def main():
     for _ in range(nprof):
         for k, v in s.profile_step().items():
             prof[k] += v / nprof
-    vol_ms = prof["vol3d"] / 5.0                                  # per launch
-    bytes_launch = algorithmic_bytes_per_element(w.N, prec) * s.K
-    flops_launch = algorithmic_flops_per_element(w.N) * s.K
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        pass
-    hbm_peak = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
-    alu_peak = FP64_TFLOPS_MEASURED if prec == 64 else FP32_TFLOPS_MEASURED
-    hbm = {"bound": "hbm", "achieved": bytes_launch / (vol_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-           "peak_source": "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback"}
-    hbm["frac"] = hbm["achieved"] / hbm["peak"]
-    alu = {"bound": "alu", "achieved": flops_launch / (vol_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
-           "peak_source": "profiles/r01_peaks.md (DFMA/FFMA microbenchmark on this pool)"}
-    alu["frac"] = alu["achieved"] / alu["peak"]
-    t_mem, t_alu = bytes_launch / (hbm_peak * 1e9), flops_launch / (alu_peak * 1e12)
-    roof = dict(hbm if t_mem >= t_alu else alu)
-    roof.update({"kernel": s.info["kernel_name"], "ms_per_launch": vol_ms, "traffic": None,
-                 "roof_ms": 1e3 * max(t_mem, t_alu), "frac_of_slower_roof": max(t_mem, t_alu) / (vol_ms * 1e-3),
-                 "hbm": hbm, "alu": alu, "kernel_share_of_step": prof["vol3d"] / max(sum(prof.values()), 1e-12),
-                 "per_kernel_ms_per_step": prof})
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")     # from the ncu --set full captures under profiles/
-    if os.path.exists(traffic_file):
-        for ln in open(traffic_file).read().splitlines()[1:]:
-            cols = ln.split(",")
-            if cols and cols[0] == f"{args.workload}_f{prec}":
-                roof["traffic"] = float(cols[1])
+    roof = roofline(s, w, prec, prof, args.workload)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the four fp64 fields, the steps, D2H of
     #      the four fields, all inside the timed region
@@ -246,20 +243,63 @@ def main():
     launches = s.launches_per_step * args.steps
     info = dict(s.info)
     s.close()
+    del s, pin_in, pin_out, host_in, host_out, q
+    torch.cuda.empty_cache()
+    return {"value": value, "ms_per_step": ms / args.steps, "roofline": roof, "e2e": e2e, "gpu_launches": launches,
+            "clocks": sampler.summary(),
+            "run": {"T": info["T"], "E": info["E"], "corners": info["C"], "dt": info["dt"], "setup_s": t_setup,
+                    "finite": finite, "kernel": info["kernel_name"], "launches_per_step": info["launches_per_step"]}}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--precision", type=int, default=64)
+    ap.add_argument("--n", type=int, default=None, help="override hexes per side (debug only; invalidates the metric)")
+    ap.add_argument("--N", type=int, default=None, help="override the polynomial degree (degree sweep of configs[3])")
+    ap.add_argument("--J", type=int, default=None, help="override the HABC order (degree sweep of configs[3])")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--kernel", type=int, default=0, help="dg_options.kernel (0 = the library's choice)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the run in the other precision")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_1610_05023_b200.replicas import Replicas
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    rep = Replicas.from_env("nccl")
+    rank, world, local = rep.rank, rep.world, rep.local
+    torch.cuda.set_device(local)
+
+    w = make_workload(args.workload, n=args.n, N=args.N, J=args.J)
+    prec = args.precision
+    first = measure(args, w, prec, rep, local)
+    line = {"metric": METRIC, "value": first["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": first["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": f"f{prec}", "data": "synthetic",
-            "config": {"workload": args.workload, "n_hex": w.n, "hex_grid": list(w.shape), "N": w.N, "J": w.J, "K": info["K"], "T": info["T"],
-                       "E": info["E"], "corners": info["C"], "nodes": nodes, "dt": info["dt"],
-                       "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "l2": "state (q,res) exceeds L2 many times over; no flush needed",
-                       "setup_s": t_setup, "finite": finite},
-            "node_stages_per_s": 5 * value, "roofline": roof, "e2e": e2e, "gpu_launches": launches,
-            "clocks": sampler.summary()}
+            "config": dict(workload_config(args.workload, w), parallelism="replicas only" if world > 1 else "single GPU",
+                           l2="state (q,res) exceeds L2 many times over; no flush needed"),
+            "run": first["run"], "node_stages_per_s": 5 * first["value"], "roofline": first["roofline"],
+            "e2e": first["e2e"], "gpu_launches": first["gpu_launches"], "clocks": first["clocks"]}
+    if not args.no_secondary:
+        # BASELINE.json's metric is quoted "(fp64/fp32)": the same workload, steps and warm-up in the other precision
+        other = 32 if prec == 64 else 64
+        sec = measure(args, w, other, rep, local)
+        line["secondary"] = {"dtype": f"f{other}", "value": sec["value"], "unit": UNIT, "ms_per_step": sec["ms_per_step"],
+                             "roofline": sec["roofline"], "e2e": sec["e2e"], "gpu_launches": sec["gpu_launches"],
+                             "clocks": sec["clocks"], "run": sec["run"]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, desc, cores, _ = oracle_sample(args.workload, prec)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        v, desc, cores, _, avail = oracle_sample(args.workload, prec)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "cores_available": avail, "kind": "oracle",
+                                "sample": desc}
     if rank == 0:
         print(json.dumps(line))
     rep.close()

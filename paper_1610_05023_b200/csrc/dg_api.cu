@@ -16,6 +16,7 @@
 #include "habc_coef.hpp"
 #include "kernels.cuh"
 #include "kernels_aux.cuh"
+#include "kernel_face2d.cuh"
 #include "kernel_vol3d_mma.cuh"
 #include "kernel_vol3d_ws.cuh"
 #include "kernel_vol3d_tf32.cuh"
@@ -78,7 +79,7 @@ struct dg_solver {
     dg::Dev<float> d32{};
     int cur = 0;
     int grid3 = 0;
-    int face_grid = 148 * 8;        // persistent CTAs of the 2D solver kernel (set from the SM count in dg_create)
+    int face_grid = 1;              // persistent CTAs of the 2D solver kernel (from the occupancy calculator, dg_create)
     size_t smem3 = 0;
     int kern3 = 0;                  // the 3D kernel in use (enum Kern3, resolved from dg_options.kernel in dg_create)
     const void* geox3 = nullptr;    // [Kp][GX3] per-tet record of the warp-specialised kernels (dt folded in), fp64 or fp32
@@ -214,7 +215,8 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     }
     d.geo3 = U.real(geo, Kp * GEO3);
     if (KERNELS[s->kern3].geox) {
-        // record of kernel_vol3d_ws.cuh: G | dt rho c^2, dt/rho, dt c | (Fs n, A)_f | B_f | Fs_f
+        // record of kernel_vol3d_ws.cuh (GX3): every scale factor of the stage folded in, Z = rho c of the cell:
+        // Ga = -dt rho c^2 G | Gb = -dt/rho G | (Fs n, Z A)_f | Z B_f | dt c Fs_f
         std::vector<double> gx;
         if (!A.dry) {
             gx.assign(Kp * GX3, 0.0);
@@ -222,13 +224,16 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
             for (int k = 0; k < K; ++k) {
                 const double* g = &geo[(size_t)k * GEO3];
                 double* x = &gx[(size_t)k * GX3];
-                for (int q = 0; q < 9; ++q) x[q] = g[q];
-                x[9] = s->dt * g[21]; x[10] = s->dt * g[22]; x[11] = s->dt * g[23];
+                const double Z = s->rho[k] * s->c[k];
+                for (int q = 0; q < 9; ++q) {
+                    x[q] = -s->dt * g[21] * g[q];
+                    x[q < 3 ? 9 + q : 33 + q] = -s->dt * g[22] * g[q];
+                }
                 for (int f = 0; f < 4; ++f) {
                     for (int c = 0; c < 3; ++c) x[12 + 4 * f + c] = NH[f][0] * g[c] + NH[f][1] * g[3 + c] + NH[f][2] * g[6 + c];
-                    x[12 + 4 * f + 3] = g[9 + f];
-                    x[28 + f] = g[13 + f];
-                    x[32 + f] = g[17 + f];
+                    x[12 + 4 * f + 3] = Z * g[9 + f];
+                    x[28 + f] = Z * g[13 + f];
+                    x[32 + f] = s->dt * g[23] * g[17 + f];
                 }
             }
         }
@@ -457,8 +462,42 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool cfg
 }
 #undef DG_CASE
 
+// 2D solver.  fp64, N <= 5: the tensor-pipe kernel (kernel_face2d.cuh); otherwise the scalar kernel.
+// configure = true: shared-memory attribute and persistent grid instead of a launch.
+template <int N>
+void face2d_mma_run(dg_solver* s, Dev<double>& d, int src, double a, double b, bool configure) {
+    using Cfg = Face2dMmaCfg<N>;
+    if (configure) {
+        cu(cudaFuncSetAttribute(k_face2d_mma<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        int per_sm = 0, sms = 0;
+        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_face2d_mma<N>, Cfg::NT, Cfg::smem_bytes), "occupancy");
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: the 2D kernel does not fit on an SM");
+        const int nitems = d.Tn * ((d.J + Cfg::SB - 1) / Cfg::SB), nchunk = (nitems + Cfg::PB - 1) / Cfg::PB;
+        s->face_grid = std::max(1, std::min(nchunk, per_sm * sms));
+        return;
+    }
+    k_face2d_mma<N><<<s->face_grid, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, a, b, s->dt);
+}
+
 template <typename T>
-void launch_face2d(dg_solver* s, Dev<T>& d, int src, double a, double b) {
+void launch_face2d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool configure = false) {
+    if constexpr (std::is_same<T, double>::value) {
+        switch (s->N) {
+            case 1: return face2d_mma_run<1>(s, d, src, a, b, configure);
+            case 2: return face2d_mma_run<2>(s, d, src, a, b, configure);
+            case 3: return face2d_mma_run<3>(s, d, src, a, b, configure);
+            case 4: return face2d_mma_run<4>(s, d, src, a, b, configure);
+            case 5: return face2d_mma_run<5>(s, d, src, a, b, configure);
+        }
+    }
+    if (configure) {
+        int sms = 0;
+        cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
+        s->face_grid = sms * 8;
+        cu(cudaFuncSetAttribute(k_face2d<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024), "smem attr");
+        return;
+    }
     const int Nf = 3 * d.N1, PB = std::max(1, FACE2D_NT / std::max(d.Nfp, Nf));
     const size_t smem = sizeof(T) * (face2d_ops_elems(d.Nfp, d.N1) + (size_t)PB * (5 * d.Nfp + Nf) * FACE2D_SB);
     const int nitems = d.Tn * ((d.J + FACE2D_SB - 1) / FACE2D_SB);
@@ -777,13 +816,6 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         const double cfl = (opt && opt->cfl > 0) ? opt->cfl : 1.0;
         s->dt = (opt && opt->dt > 0) ? opt->dt : cfl * dtmin;
         cu(cudaSetDevice(s->device), "cudaSetDevice");
-        {
-            int sms = 0;
-            cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-            s->face_grid = sms * 8;
-            cu(cudaFuncSetAttribute(k_face2d<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024), "smem attr");
-            cu(cudaFuncSetAttribute(k_face2d<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024), "smem attr");
-        }
         const size_t need = dry_bytes(s);
         if (opt && opt->workspace_dev) {
             if (opt->workspace_bytes < need) throw std::runtime_error("ENOMEM: workspace_bytes is smaller than dg_workspace_bytes");
@@ -797,8 +829,15 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         // align the arena base to 256 B
         size_t mis = (size_t)(uintptr_t)A.base & 255;
         if (mis) { A.base += 256 - mis; A.size -= 256 - mis; }
-        if (precision == 64) { build_device<double>(s, A, s->d64); launch_vol3d<double>(s, s->d64, 0, 0, 0, true); }
-        else { build_device<float>(s, A, s->d32); launch_vol3d<float>(s, s->d32, 0, 0, 0, true); }
+        if (precision == 64) {
+            build_device<double>(s, A, s->d64);
+            launch_vol3d<double>(s, s->d64, 0, 0, 0, true);
+            if (s->d64.J > 0 && s->d64.Tn > 0) launch_face2d<double>(s, s->d64, 0, 0, 0, true);
+        } else {
+            build_device<float>(s, A, s->d32);
+            launch_vol3d<float>(s, s->d32, 0, 0, 0, true);
+            if (s->d32.J > 0 && s->d32.Tn > 0) launch_face2d<float>(s, s->d32, 0, 0, 0, true);
+        }
         cu(cudaDeviceSynchronize(), "setup");
         *out = s;
         return DG_OK;

@@ -38,7 +38,7 @@ struct TfCfg {
     static constexpr int NT = 384;
     static constexpr int NS = 3;                       // staging depth
     static constexpr int QS = Np * 4 + 4;              // staged element stride of q / res in floats (16 B skew)
-    static constexpr int GS = GX3 + 4;                 // staged stride of the record (176 B)
+    static constexpr int GS = GX3 + 8;                 // staged stride of the record (208 B = 13 x 16 B: bank spread)
     static constexpr int szB = (4 * KPD + 4 * KPL) * XS;
     static constexpr int oB = 0;                       // [2][szB]        operand buffers
     static constexpr int oQ = oB + 2 * szB;            // [NS][16][QS]
@@ -311,23 +311,24 @@ k_vol3d_tf32(Dev<float> d, const float* __restrict__ geox, int src, float rka, f
             const int e = g + 8 * r;
             if (e0 + e < K) {
                 const float* ge = sGeo + (s * EB + e) * GS;
-                const float4 ga = *reinterpret_cast<const float4*>(ge), gb = *reinterpret_cast<const float4*>(ge + 4),
-                             gc = *reinterpret_cast<const float4*>(ge + 8), fs = *reinterpret_cast<const float4*>(ge + 32);
-                const float g8 = gc.x, rc2 = gc.y, irho = gc.z, cc = gc.w;      // material constants already times dt
+                // the record carries every scale factor (GX3 in kernel_vol3d_ws.cuh): Gb = -dt/rho G at 9..11, 36..41
+                const float4 gc = *reinterpret_cast<const float4*>(ge + 8), gd = *reinterpret_cast<const float4*>(ge + 36),
+                             fs = *reinterpret_cast<const float4*>(ge + 32);
+                const float2 ge2 = *reinterpret_cast<const float2*>(ge + 40);
+                const float b0 = gc.y, b1 = gc.z, b2 = gc.w, b3 = gd.x, b4 = gd.y, b5 = gd.z, b6 = gd.w, b7 = ge2.x, b8 = ge2.y;
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     const int n = 8 * w + 2 * t + c, i = 2 * r + c;
                     if (n < Np) {
                         const float a0 = cl[0][i], a1 = cl[1][i], a2 = cl[2][i], a3 = cl[3][i];
-                        const float lp = fs.x * a0 + fs.y * a1 + fs.z * a2 + fs.w * a3;
-                        // -1/rho grad p + c * sum_f (Fs n)_f LIFT_f g, both through G^T:  G^T (c*l - irho*dp)
-                        const float xr = cc * (a2 - a3) - irho * cpr[i];
-                        const float xs = cc * (a2 - a1) - irho * cps[i];
-                        const float xt = cc * (a2 - a0) - irho * cpt[i];
-                        const float rp = -rc2 * (cdv[i] + lp);
-                        const float ru = ga.x * xr + ga.w * xs + gb.z * xt;
-                        const float rv = ga.y * xr + gb.x * xs + gb.w * xt;
-                        const float rw = ga.z * xr + gb.y * xs + g8 * xt;
+                        // accumulators: -dt rho c^2 div u, D p, Z LIFT_f g; the reference normals combine the lifts
+                        const float yr = (cpr[i] - a2) + a3;
+                        const float ys = (cps[i] - a2) + a1;
+                        const float yt = (cpt[i] - a2) + a0;
+                        const float rp = (((cdv[i] - fs.x * a0) - fs.y * a1) - fs.z * a2) - fs.w * a3;
+                        const float ru = b0 * yr + b3 * ys + b6 * yt;
+                        const float rv = b1 * yr + b4 * ys + b7 * yt;
+                        const float rw = b2 * yr + b5 * ys + b8 * yt;
                         float4 q = *reinterpret_cast<const float4*>(sQ + (s * EB + e) * QS + n * 4);
                         float4 rr = *reinterpret_cast<const float4*>(sR + (s * EB + e) * QS + n * 4);
                         rr.x = rka * rr.x + rp;  q.x += rkb * rr.x;

@@ -20,10 +20,12 @@
 
 namespace dg {
 
-constexpr int GX3 = 40;   // per-tet record of this kernel, in doubles:
-                          //  0..8  G = (r,s,t)_(x,y,z)        9 dt*rho*c^2   10 dt/rho   11 dt*c
-                          // 12+4f  (Fs n)_x, (Fs n)_y, (Fs n)_z, A_f   (f = 0..3; scaled OUTWARD normal)
-                          // 28+f   B_f            32+f  Fs_f          36..39 pad
+constexpr int GX3 = 44;   // per-tet record of this kernel, in values of T.  Every constant of the stage is folded in on
+                          // the host, so that the update needs no scaling of its own (Z = rho c of the cell):
+                          //  0..8   Ga = -dt rho c^2 G, G = (r,s,t)_(x,y,z): the operand rows are -dt rho c^2 (G u)
+                          //  9..11, 36..41  Gb = -dt/rho G: the velocity right-hand side is Gb^T y
+                          // 12+4f   (Fs n)_x, (Fs n)_y, (Fs n)_z, Z A_f   (f = 0..3; scaled OUTWARD normal)
+                          // 28+f    Z B_f          32+f  dt c Fs_f          42, 43 pad
                           // A_f = Z+/((Z+ + Z-) Fs_f), B_f = 1/(Z+ + Z-)   (upwind flux)
 
 template <int N>
@@ -41,8 +43,8 @@ struct WsCfg {
     // (8 elements, one node per quarter-warp) and the update of the MMA warps (4 elements of equal parity x 2
     // adjacent nodes per quarter-warp: elements {0,2,4,6} -> slots {0,1,4,5}, {1,3,5,7} -> {2,3,6,7})
     static constexpr int QS = ((Np * 4 + 15) / 16) * 16 + 16;
-    static constexpr int GS = GX3 + 2;                 // staged stride of the geometric record: 336 B, so that the
-                                                       // records of elements 0,2,4,6 (and 0..7) fall in distinct banks
+    static constexpr int GS = GX3 + 2;                 // staged stride of the geometric record: 368 B = 23 x 16 B, so that
+                                                       // the records of elements 0..7 fall in distinct 16-byte bank groups
     static constexpr int szB = 4 * KPD * EB + 4 * LPAD;
     static constexpr int oB = 0;                       // [2][szB]        operand buffers
     static constexpr int oQ = oB + 2 * szB;            // [NS][8][QS]
@@ -301,21 +303,20 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
                 const int e = 2 * t + ee;
                 if (e0 + e < K) {
                     const double* ge = bgeo + e * GS;
-                    const double2 g01 = *reinterpret_cast<const double2*>(ge), g23 = *reinterpret_cast<const double2*>(ge + 2),
-                                  g45 = *reinterpret_cast<const double2*>(ge + 4), g67 = *reinterpret_cast<const double2*>(ge + 6),
-                                  g8r = *reinterpret_cast<const double2*>(ge + 8), irc = *reinterpret_cast<const double2*>(ge + 10),
+                    const double2 b01 = *reinterpret_cast<const double2*>(ge + 8), b12 = *reinterpret_cast<const double2*>(ge + 10),
+                                  b34 = *reinterpret_cast<const double2*>(ge + 36), b56 = *reinterpret_cast<const double2*>(ge + 38),
+                                  b78 = *reinterpret_cast<const double2*>(ge + 40),
                                   f01 = *reinterpret_cast<const double2*>(ge + 32), f23 = *reinterpret_cast<const double2*>(ge + 34);
                     const double a0 = cl[0][ee], a1 = cl[1][ee], a2 = cl[2][ee], a3 = cl[3][ee];
-                    const double lp = f01.x * a0 + f01.y * a1 + f23.x * a2 + f23.y * a3;
-                    const double rc2 = g8r.y, irho = irc.x, cc = irc.y;        // each already times dt
-                    // -1/rho grad p + c * sum_f (Fs n)_f LIFT_f g, both through G^T:  G^T (c*l - irho*dp)
-                    const double xr = cc * (a2 - a3) - irho * cpr[ee];
-                    const double xs = cc * (a2 - a1) - irho * cps[ee];
-                    const double xt = cc * (a2 - a0) - irho * cpt[ee];
-                    const double rp = -rc2 * ((cvr[ee] + cvs[ee]) + cvt[ee] + lp);
-                    const double ru = g01.x * xr + g23.y * xs + g67.x * xt;
-                    const double rv = g01.y * xr + g45.x * xs + g67.y * xt;
-                    const double rw = g23.x * xr + g45.y * xs + g8r.x * xt;
+                    // the record carries every scale factor (GX3 above): the accumulators are -dt rho c^2 div u,
+                    // D p and Z LIFT_f g; the reference normals (0,0,-1), (0,-1,0), (1,1,1), (-1,0,0) combine the lifts
+                    const double yr = (cpr[ee] - a2) + a3;
+                    const double ys = (cps[ee] - a2) + a1;
+                    const double yt = (cpt[ee] - a2) + a0;
+                    const double rp = (((((cvr[ee] + cvs[ee]) + cvt[ee]) - f01.x * a0) - f01.y * a1) - f23.x * a2) - f23.y * a3;
+                    const double ru = b01.y * yr + b34.x * ys + b56.y * yt;       // Gb^T y: Gb[0], Gb[3], Gb[6]
+                    const double rv = b12.x * yr + b34.y * ys + b78.x * yt;       //         Gb[1], Gb[4], Gb[7]
+                    const double rw = b12.y * yr + b56.x * ys + b78.y * yt;       //         Gb[2], Gb[5], Gb[8]
                     const int eo = ws_eoff(e, QS) + n * 4;
                     double2 q0 = *reinterpret_cast<const double2*>(bq + eo);
                     double2 q1 = *reinterpret_cast<const double2*>(bq + eo + 2);
