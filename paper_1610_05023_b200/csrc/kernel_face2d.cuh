@@ -40,13 +40,21 @@ struct Face2dMmaCfg {
     static constexpr int oRaw = ROWS * RS;
     static constexpr int oRes = oRaw + PB * RAW;
     static constexpr int oIc = oRes + NRES * NT;
-    static constexpr size_t smem_bytes = sizeof(double) * (oIc + 16);
+    // per-item records staged with the fields (double-buffered: phases 2 and 3 still read them while the next chunk's
+    // arrive): geo2 [24] | S2 row [Nfp, padded to even] | ints: nbr2 [3], nbrnode2 [3][N1]
+    static constexpr int mS = GEO2, mI = mS + Nfp + (Nfp & 1), NMI = 3 + Nf, META = mI + (NMI + 1) / 2 + ((NMI + 1) / 2 & 1);
+    static constexpr int oMeta = oIc + 16;
+    static constexpr size_t smem_bytes = sizeof(double) * (oMeta + 2 * PB * META);
+    static_assert(GEO2 / 2 + Nfp + NMI <= 64, "metadata copy units per item");
     static constexpr int regsA = 2 * MT * (2 * KD + 3 * KL);
     static_assert(regsA <= 150, "operator fragments do not fit the register file: use k_face2d");
 };
 
 __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int NKEEP> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NKEEP) : "memory"); }
@@ -61,6 +69,8 @@ __global__ void __launch_bounds__(Face2dMmaCfg<N>::NT, 2) k_face2d_mma(Dev<doubl
     double* sRaw = sOp + C::oRaw;                          // [PB][4][3][Nfp]
     double* sRes = sOp + C::oRes;                          // [NRES][NT]: lane-private residual values
     double* sIc = sOp + C::oIc;                            // [J] 1 / (1 + c_i)   (eq (31a))
+    double* sMeta = sOp + C::oMeta;                        // [2][PB][META]
+    constexpr int META = C::META;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, t = lane & 3;
     const int J = d.J;
     const int NG = (J + SB - 1) / SB;                      // set groups per triangle
@@ -92,9 +102,21 @@ __global__ void __launch_bounds__(Face2dMmaCfg<N>::NT, 2) k_face2d_mma(Dev<doubl
             }
     }
 
-    // raw fields of a chunk -> sRaw (set q of item pl at [pl][q][field][node]); sets beyond J read as zero
-    auto issue_fields = [&](int chunk_) {
+    // raw fields of a chunk -> sRaw (set q of item pl at [pl][q][field][node]); sets beyond J read as zero;
+    // the items' records (geometry, closure S of the triangle, neighbour tables) -> sMeta[buf]
+    auto issue_fields = [&](int chunk_, int buf) {
         if (chunk_ >= nchunk) return;
+        for (int u = tid; u < PB * 64; u += NT) {
+            const int pl = u >> 6, k = u & 63, item = chunk_ * PB + pl;
+            if (item >= nitems) continue;
+            const int tt = item / NG;
+            double* mt = sMeta + (buf * PB + pl) * META;
+            if (k < GEO2 / 2) cp_async16(mt + 2 * k, d.geo2 + (size_t)tt * GEO2 + 2 * k);
+            else if (k < GEO2 / 2 + Nfp) cp_async8(mt + C::mS + (k - GEO2 / 2), d.S2 + (size_t)tt * Nfp + (k - GEO2 / 2));
+            else if (k < GEO2 / 2 + Nfp + 3) cp_async4(reinterpret_cast<int*>(mt + C::mI) + (k - GEO2 / 2 - Nfp), d.nbr2 + tt * 3 + (k - GEO2 / 2 - Nfp));
+            else if (k < GEO2 / 2 + Nfp + C::NMI)
+                cp_async4(reinterpret_cast<int*>(mt + C::mI) + (k - GEO2 / 2 - Nfp), d.nbrnode2 + (size_t)tt * Nf + (k - GEO2 / 2 - Nfp - 3));
+        }
         for (int u = tid; u < PB * Nfp; u += NT) {
             const int pl = u / Nfp, n = u - pl * Nfp, item = chunk_ * PB + pl;
             if (item >= nitems) continue;
@@ -113,9 +135,10 @@ __global__ void __launch_bounds__(Face2dMmaCfg<N>::NT, 2) k_face2d_mma(Dev<doubl
     // the accumulator fragment of lane (g, t) holds columns 2t, 2t+1 of the warp's n-tile: item pl3, sets q0, q0 + 1
     const int pl3 = 2 * wid + (t >> 1), q0 = 2 * (t & 1), col3 = 8 * wid + 2 * t;
 
-    issue_fields(blockIdx.x);
+    issue_fields(blockIdx.x, 0);
     cp_async_commit();
-    for (int chunk = blockIdx.x; chunk < nchunk; chunk += gridDim.x) {
+    int par = 0;
+    for (int chunk = blockIdx.x; chunk < nchunk; chunk += gridDim.x, par ^= 1) {
         cp_async_wait<0>();
         __syncthreads();                                   // this chunk's raw fields are in; the operand rows are free
         // ---- residual values of this lane: land under phases 1-3
@@ -137,9 +160,8 @@ __global__ void __launch_bounds__(Face2dMmaCfg<N>::NT, 2) k_face2d_mma(Dev<doubl
         for (int u = tid; u < PB * Nfp; u += NT) {
             const int pl = u / Nfp, n = u - pl * Nfp, item = chunk * PB + pl;
             if (item >= nitems) continue;
-            const int tt = item / NG;
-            const double* gg = d.geo2 + (size_t)tt * GEO2;   // G2 = (r_xi, r_eta, s_xi, s_eta) | n[3][2] | ...
-            const double S = d.S2[(size_t)tt * Nfp + n];
+            const double* gg = sMeta + (par * PB + pl) * META;   // G2 = (r_xi, r_eta, s_xi, s_eta) | n[3][2] | ...
+            const double S = gg[C::mS + n];
             const double g0 = gg[0], g1 = gg[1], g2 = gg[2], g3 = gg[3];
             const double* r = sRaw + pl * RAW + n;
             double ps[SB], uu[SB], vv[SB], pp[SB], ur[SB], us[SB];
@@ -155,18 +177,19 @@ __global__ void __launch_bounds__(Face2dMmaCfg<N>::NT, 2) k_face2d_mma(Dev<doubl
             st4<double>(mrow + C::rU * RS, uu); st4<double>(mrow + C::rV * RS, vv); st4<double>(mrow + C::rQ * RS, ps);
         }
         __syncthreads();
-        issue_fields(chunk + gridDim.x);                   // the raw buffer is free again
+        issue_fields(chunk + gridDim.x, par ^ 1);          // the raw buffer is free again
         cp_async_commit();
         // ---- phase 2: flux jump at edge node (e, m) of the triangle
         for (int u = tid; u < PB * Nf; u += NT) {
             const int pl = u / Nf, n = u - pl * Nf, item = chunk * PB + pl;
             if (item >= nitems) continue;
             const int tt = item / NG, i0 = (item - tt * NG) * SB, ns = min(SB, J - i0);
-            const double* gg = d.geo2 + (size_t)tt * GEO2;
+            const double* gg = sMeta + (par * PB + pl) * META;
+            const int* gi = reinterpret_cast<const int*>(gg + C::mI);
             const int e = n / N1, m = n - e * N1;
             const int a = d.fmask2[n];
-            const int nb = d.nbr2[tt * 3 + e];
-            const int bnode = d.nbrnode2[(tt * 3 + e) * N1 + m];
+            const int nb = gi[e];
+            const int bnode = gi[3 + n];
             const double nxe = gg[4 + 2 * e], nye = gg[5 + 2 * e], Ae = gg[13 + e], Be = gg[16 + e];
             const double* mo = sOp + a * RS + pl * SB;
             double pM[SB], uM[SB], vM[SB], gj[SB];
@@ -194,7 +217,7 @@ __global__ void __launch_bounds__(Face2dMmaCfg<N>::NT, 2) k_face2d_mma(Dev<doubl
         }
         __syncthreads();
         // ---- phase 3: contractions (DMMA), right-hand side and LSRK update from the accumulator fragments
-        const double* gg = d.geo2 + (size_t)t3 * GEO2;
+        const double* gg = sMeta + (par * PB + pl3) * META;
         const double g0 = gg[0], g1 = gg[1], g2 = gg[2], g3 = gg[3];
         const double rc2 = gg[19], irho = gg[20], cc_ = gg[21];
         const double fs0 = gg[10], fs1 = gg[11], fs2 = gg[12];
