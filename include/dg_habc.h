@@ -145,7 +145,25 @@ int dg_mesh_counts(const dg_mesh* mesh, const int32_t* face_bc, int32_t* counts)
  * ms[0..5] = volume+surface+update 3D, 2D update, 1D update, face closure, edge closure, corner closure. */
 int dg_profile_step(dg_solver* s, double* ms);
 
+/* Raw device pointers of the current state, in the library's own layout (optional, lets a caller read
+ * traces or fields on the device without the fp64 host round trip of dg_get_fields).  The pointers stay owned by the
+ * library, are valid until dg_destroy, and hold the state reached by the work already enqueued on the solver's stream
+ * (the caller orders its own reads after that stream).  dg_step flips the ping-pong buffers: call again after it.
+ * elem_bytes = 8 (fp64) or 4 (fp32).  Layouts: q [K][Np][4] = (p,u,v,w) per node; face_aux [T][J][3][Nfp] holds the
+ * ODE state p*_i and the two tangential velocities, and face_S [T][Nfp] the closure sum S = r^- + r^+ with
+ * p_i00 = p*_i + S (eq (29)); edge_aux [E][J*J][2][N+1] holds p*_ij and the tangential velocity. */
+typedef struct {
+    int32_t elem_bytes;
+    int32_t reserved;
+    const void* q;
+    const void* face_aux;
+    const void* face_S;
+    const void* edge_aux;
+} dg_device_view;
+int dg_get_device_ptrs(const dg_solver* s, dg_device_view* out);
+
 const char* dg_last_error(void);
+/* Waits for the solver's stream, then frees what the library owns (never the caller's workspace). */
 void dg_destroy(dg_solver* s);
 
 #ifdef __cplusplus

@@ -34,9 +34,14 @@ class _Info(C.Structure):
                 ("kernel", C.c_int32), ("kernel_name", C.c_char * 44)]
 
 
+class _DeviceView(C.Structure):
+    _fields_ = [("elem_bytes", C.c_int32), ("reserved", C.c_int32), ("q", C.c_void_p), ("face_aux", C.c_void_p),
+                ("face_S", C.c_void_p), ("edge_aux", C.c_void_p)]
+
+
 EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_set_source", "dg_step",
            "dg_get_fields", "dg_get_face_map", "dg_get_edge_map", "dg_reference_element", "dg_mesh_counts",
-           "dg_profile_step", "dg_last_error", "dg_destroy"]
+           "dg_profile_step", "dg_get_device_ptrs", "dg_last_error", "dg_destroy"]
 
 
 def lib() -> C.CDLL:
@@ -186,6 +191,14 @@ class Solver:
         ea = np.zeros((self.E, self.J * self.J, 2, self.N + 1)) if aux else None
         _check(lib().dg_get_fields(self._h, _dp(q[0]), _dp(q[1]), _dp(q[2]), _dp(q[3]), _dp(fa), _dp(ea)))
         return q, fa, ea
+
+    def device_view(self):
+        """dg_get_device_ptrs: raw device addresses of the current state in the library's layout (q [K][Np][4], face
+        auxiliary state [T][J][3][Nfp] + closure sum S [T][Nfp], edge auxiliary state [E][J*J][2][N+1]) and the element
+        size in bytes.  Valid until the next step() flips the buffers; order reads after `self.stream`."""
+        v = _DeviceView()
+        _check(lib().dg_get_device_ptrs(self._h, C.byref(v)))
+        return {k: getattr(v, k) for k, _ in _DeviceView._fields_ if k != "reserved"}
 
     def get_face_map(self):
         tet, face, axis, sign = (np.empty(self.T, dtype=np.int32) for _ in range(4))

@@ -1015,6 +1015,24 @@ int dg_get_edge_map(const dg_solver* s, int32_t* axis, int32_t* normal_axes, int
     return DG_OK;
 }
 
+int dg_get_device_ptrs(const dg_solver* s, dg_device_view* o) {
+    if (!s || !o) return set_err(DG_EINVAL, "EINVAL: NULL argument");
+    const bool aux = s->J > 0;
+    o->reserved = 0;
+    if (s->precision == 64) {
+        const dg::Dev<double>& d = s->d64;
+        o->elem_bytes = 8; o->q = d.q[s->cur];
+        o->face_aux = aux && d.Tn > 0 ? d.fa[s->cur] : nullptr; o->face_S = aux && d.Tn > 0 ? d.S2 : nullptr;
+        o->edge_aux = aux && d.E > 0 ? d.ea[s->cur] : nullptr;
+    } else {
+        const dg::Dev<float>& d = s->d32;
+        o->elem_bytes = 4; o->q = d.q[s->cur];
+        o->face_aux = aux && d.Tn > 0 ? d.fa[s->cur] : nullptr; o->face_S = aux && d.Tn > 0 ? d.S2 : nullptr;
+        o->edge_aux = aux && d.E > 0 ? d.ea[s->cur] : nullptr;
+    }
+    return DG_OK;
+}
+
 int dg_profile_step(dg_solver* s, double* ms) {
     try {
         if (!s || !ms) throw std::runtime_error("EINVAL: NULL argument");

@@ -214,6 +214,41 @@ def test_edge_cases():
     s.close()
 
 
+@pytest.mark.parametrize("prec", [64, 32])
+def test_device_view_matches_get_fields(prec):
+    """dg_get_device_ptrs (optional): the raw device state read through the exported pointers and the
+    documented layouts is what dg_get_fields returns (p_i00 = p*_i + S, eq (29))."""
+    import torch
+    from cuda.bindings import runtime as cudart
+    from paper_1610_05023_b200 import Solver
+    w = make_workload("cfg1", n=2, N=3, J=2, nsteps=7)
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec)
+    x, y, z = s.get_nodes()
+    s.set_initial(*parity.initial_on(w, x, y, z, w.c, w.rho))
+    s.step(7)
+    q, fa, ea = s.get_fields()
+    v = s.device_view()
+    assert v["elem_bytes"] == prec // 8
+    dt = torch.float64 if prec == 64 else torch.float32
+
+    def view(ptr, n):
+        t = torch.empty(n, dtype=dt, device="cuda")
+        s.stream.synchronize()
+        err, = cudart.cudaMemcpy(t.data_ptr(), ptr, n * v["elem_bytes"], cudart.cudaMemcpyKind.cudaMemcpyDeviceToDevice)
+        assert int(err) == 0
+        return t.cpu().double().numpy()
+
+    qd = view(v["q"], s.K * s.Np * 4).reshape(s.K, s.Np, 4)
+    assert np.array_equal(qd.transpose(2, 0, 1), q)
+    fd = view(v["face_aux"], s.T * s.J * 3 * s.Nfp).reshape(s.T, s.J, 3, s.Nfp)
+    S = view(v["face_S"], s.T * s.Nfp).reshape(s.T, 1, s.Nfp)
+    assert np.array_equal(fd[:, :, 1:], fa[:, :, 1:])
+    assert np.abs(fd[:, :, 0] + S - fa[:, :, 0]).max() <= 4 * np.finfo(np.float64 if prec == 64 else np.float32).eps * np.abs(fa[:, :, 0]).max()
+    ed = view(v["edge_aux"], s.E * s.J * s.J * 2 * (s.N + 1)).reshape(s.E, s.J * s.J, 2, s.N + 1)
+    assert np.array_equal(ed[:, :, 1], ea[:, :, 1])
+    s.close()
+
+
 def test_missing_device_is_loud(monkeypatch):
     import torch
     from paper_1610_05023_b200 import DgError, Solver
