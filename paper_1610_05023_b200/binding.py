@@ -93,7 +93,7 @@ def dg_reference_element(dim: int, N: int):
 
 _BC_CODES = {"habc": 0, "dirichlet": 1, "rigid": 2}
 # dg_options.kernel (DG_KERNEL_* of include/dg_habc.h)
-KERNEL_AUTO, KERNEL_SCALAR, KERNEL_MMA, KERNEL_WS, KERNEL_TF32, KERNEL_TPG = range(6)
+KERNEL_AUTO, KERNEL_SCALAR, KERNEL_MMA, KERNEL_WS, KERNEL_TF32, KERNEL_TPG, KERNEL_ELEM = range(7)
 
 
 def _face_bc_codes(face_bc):

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdg_habc.so")
 SOURCES = ["dg_api.cu", "mesh.cpp", "refelem.cpp"]
-HEADERS = ["kernels.cuh", "kernels_aux.cuh", "kernel_face2d.cuh", "kernel_vol3d_mma.cuh", "kernel_vol3d_ws.cuh", "kernel_vol3d_tf32.cuh", "kernel_vol3d_mmag.cuh", "kernel_vol3d_tf32g.cuh", "mesh.hpp", "refelem.hpp", "habc_coef.hpp",
+HEADERS = ["kernels.cuh", "kernels_aux.cuh", "kernel_face2d.cuh", "kernel_vol3d_mma.cuh", "kernel_vol3d_ws.cuh", "kernel_vol3d_tf32.cuh", "kernel_vol3d_mmag.cuh", "kernel_vol3d_tf32g.cuh", "kernel_vol3d_elem.cuh", "mesh.hpp", "refelem.hpp", "habc_coef.hpp",
            os.path.join("..", "..", "include", "dg_habc.h")]
 
 

@@ -22,6 +22,7 @@
 #include "kernel_vol3d_tf32.cuh"
 #include "kernel_vol3d_mmag.cuh"
 #include "kernel_vol3d_tf32g.cuh"
+#include "kernel_vol3d_elem.cuh"
 #include "mesh.hpp"
 
 namespace {
@@ -104,7 +105,7 @@ using namespace dg;
 
 // The 3D kernels.  The values are dg_options.kernel (include/dg_habc.h); KERNELS says what each one covers and
 // DEFAULT_KERNEL which one runs when the caller asks for 0.
-enum Kern3 : int { K3_AUTO = 0, K3_SCALAR = 1, K3_MMA = 2, K3_WS = 3, K3_TF32 = 4, K3_TPG = 5, K3_COUNT };
+enum Kern3 : int { K3_AUTO = 0, K3_SCALAR = 1, K3_MMA = 2, K3_WS = 3, K3_TF32 = 4, K3_TPG = 5, K3_ELEM = 6, K3_COUNT };
 
 struct KernRow { int precision /* 0: both */, nmin, nmax; bool geox /* reads the extended per-tet record */; const char* what; };
 const KernRow KERNELS[K3_COUNT] = {
@@ -114,13 +115,14 @@ const KernRow KERNELS[K3_COUNT] = {
     {64, 4, 5, true, "warp-specialised fp64 tensor-pipe kernel (kernel = 3): fp64, N = 4, 5"},
     {32, 3, 5, true, "fp32 3xTF32 tensor-core kernel (kernel = 4): fp32, N = 3..5"},
     {0, 6, 8, false, "tensor-pipe kernels with operators read through L1/L2 (kernel = 5): N = 6..8"},
+    {32, 1, 2, false, "thread-per-element fp32 kernel (kernel = 6): fp32, N = 1, 2"},
 };
 //                                    N =      1          2          3        4        5      6       7       8
 const int DEFAULT_KERNEL_F64[9] = {0, K3_MMA,    K3_MMA,    K3_MMA,  K3_MMA,  K3_WS,   K3_TPG, K3_TPG, K3_TPG};
-const int DEFAULT_KERNEL_F32[9] = {0, K3_SCALAR, K3_SCALAR, K3_TF32, K3_TF32, K3_TF32, K3_TPG, K3_TPG, K3_TPG};
+const int DEFAULT_KERNEL_F32[9] = {0, K3_ELEM,   K3_ELEM,   K3_TF32, K3_TF32, K3_TF32, K3_TPG, K3_TPG, K3_TPG};
 
 int resolve_kernel(int requested, int precision, int N) {
-    if (requested < 0 || requested >= K3_COUNT) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..5");
+    if (requested < 0 || requested >= K3_COUNT) throw std::runtime_error("EINVAL: dg_options.kernel must be 0..6");
     const int k = requested != K3_AUTO ? requested : (precision == 64 ? DEFAULT_KERNEL_F64 : DEFAULT_KERNEL_F32)[N];
     const KernRow& r = KERNELS[k];
     if ((r.precision && r.precision != precision) || N < r.nmin || N > r.nmax)
@@ -212,6 +214,15 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
         for (int n = 0; n < Np; ++n)
             for (int j = 0; j < 4 * Nfp; ++j) lt3[(size_t)j * Np + n] = m.r3.LIFT[(size_t)n * 4 * Nfp + j];
         fm3.assign(m.r3.Fmask.begin(), m.r3.Fmask.end());
+    }
+    if (!A.dry && m.N <= ELEM_MAXN && std::is_same<T, float>::value) {
+        // k_vol3d_elem reads its operators from constant memory: D[3][Np][Np] | LIFT[Np][4 Nfp], one slot per degree
+        // (the values depend on N only, so solvers of the same degree write the same bytes)
+        std::vector<float> ops((size_t)3 * Np * Np + (size_t)Np * 4 * Nfp);
+        for (int a = 0; a < 3; ++a)
+            for (size_t i = 0; i < (size_t)Np * Np; ++i) ops[(size_t)a * Np * Np + i] = (float)m.r3.D[a][i];
+        for (size_t i = 0; i < (size_t)Np * 4 * Nfp; ++i) ops[(size_t)3 * Np * Np + i] = (float)m.r3.LIFT[i];
+        cu(cudaMemcpyToSymbol(c_elem_ops, ops.data(), sizeof(float) * ops.size(), sizeof(float) * (size_t)(m.N - 1) * ELEM_OPS), "upload operators");
     }
     d.geo3 = U.real(geo, Kp * GEO3);
     if (KERNELS[s->kern3].geox) {
@@ -407,6 +418,18 @@ void vol3d_tf32g(dg_solver* s, Dev<float>& d, int src, double a, double b, bool 
     run_vol3d(s, k_vol3d_tf32g<N, W>, Cfg::NT, Cfg::smem_bytes, Cfg::EPB, d.K, false, cfg, d, src, (float)a, (float)b, (float)s->dt);
 }
 
+template <int N>
+void vol3d_elem(dg_solver* s, Dev<float>& d, int src, double a, double b, bool cfg) {
+    using Cfg = ElemCfg<N>;
+    if (cfg) {
+        cu(cudaFuncSetAttribute(k_vol3d_elem<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes), "smem attr");
+        s->grid3 = std::max(1, (d.K + Cfg::NT - 1) / Cfg::NT);     // one thread per element, not persistent
+        s->smem3 = Cfg::smem_bytes;
+        return;
+    }
+    k_vol3d_elem<N><<<s->grid3, Cfg::NT, Cfg::smem_bytes, s->stream>>>(d, src, (float)a, (float)b, (float)s->dt);
+}
+
 template <typename T> struct OpsFit;                         // scalar kernel: degrees whose operators fit shared memory
 template <> struct OpsFit<double> { static constexpr int maxN = 5; };
 template <> struct OpsFit<float> { static constexpr int maxN = 6; };
@@ -446,6 +469,11 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool cfg
             if constexpr (!F64) switch (N) {
                 DG_CASE(3, vol3d_tf32<3>(s, d, src, a, b, cfg)); DG_CASE(4, vol3d_tf32<4>(s, d, src, a, b, cfg));
                 DG_CASE(5, vol3d_tf32<5>(s, d, src, a, b, cfg));
+            }
+            break;
+        case K3_ELEM:
+            if constexpr (!F64) switch (N) {
+                DG_CASE(1, vol3d_elem<1>(s, d, src, a, b, cfg)); DG_CASE(2, vol3d_elem<2>(s, d, src, a, b, cfg));
             }
             break;
         case K3_TPG:
@@ -864,7 +892,7 @@ int dg_get_info(const dg_solver* s, dg_info* o) {
     o->dt = s->dt; o->device_bytes = s->ws_bytes;
     o->kernel = s->kern3;
     static const char* const NAMES[K3_COUNT][2] = {{"", ""}, {"k_vol3d", "k_vol3d"}, {"k_vol3d_mma", ""}, {"k_vol3d_ws", ""},
-                                                   {"", "k_vol3d_tf32"}, {"k_vol3d_mmag", "k_vol3d_tf32g"}};
+                                                   {"", "k_vol3d_tf32"}, {"k_vol3d_mmag", "k_vol3d_tf32g"}, {"", "k_vol3d_elem"}};
     snprintf(o->kernel_name, sizeof(o->kernel_name), "%s<%d>", NAMES[s->kern3][s->precision == 32], s->N);
     return DG_OK;
 }

@@ -77,9 +77,10 @@ def test_3d_kernel_variants(N, kernel):
     _check(parity.compare(lib, ora), 64)
 
 
-@pytest.mark.parametrize("N,kernel", [(3, 4), (4, 4), (5, 4), (1, 1), (3, 1), (5, 1), (5, 0), (6, 5), (7, 5), (8, 5), (6, 1)])
+@pytest.mark.parametrize("N,kernel", [(3, 4), (4, 4), (5, 4), (1, 1), (2, 1), (1, 6), (2, 6), (3, 1), (5, 1), (5, 0), (6, 5), (7, 5), (8, 5), (6, 1)])
 def test_3d_kernel_variants_fp32(N, kernel):
-    """fp32: 1 scalar FMA, 4 / 5 tensor cores with 3xTF32 error compensation (N = 3..5 / N = 6..8) -- all inside the
+    """fp32: 1 scalar FMA, 6 one thread per element (N = 1, 2), 4 / 5 tensor cores with 3xTF32 error compensation
+    (N = 3..5 / N = 6..8) -- all inside the
     fp32 tolerance, and the compensated tensor-core result no worse than 4x the FMA kernel's error.
     750 tets = 46 batches of 16 + a ragged tail of 14."""
     w = make_workload("cfg5", n=5, N=N, J=3, nsteps=12)
@@ -95,7 +96,7 @@ def test_kernel_choice_is_validated():
     """a kernel that does not cover (precision, N) is refused with DG_EINVAL, not silently replaced"""
     from paper_1610_05023_b200 import DgError, Solver
     w = make_workload("cfg1")
-    for N, prec, kernel in ((6, 64, 2), (3, 64, 3), (5, 64, 4), (2, 32, 4), (5, 32, 5), (3, 64, 6), (3, 64, -1)):
+    for N, prec, kernel in ((6, 64, 2), (3, 64, 3), (5, 64, 4), (2, 32, 4), (5, 32, 5), (3, 32, 6), (2, 64, 6), (3, 64, 7), (3, 64, -1)):
         with pytest.raises(DgError):
             Solver(w.verts, w.tets, N, 2, w.c, w.rho, precision=prec, kernel=kernel)
 
