@@ -254,6 +254,51 @@ void build_device(dg_solver* s, Arena& A, Dev<T>& d) {
     d.finfo3 = U.template ints<uint32_t>(finfo, K);
     d.conn3 = U.template ints<uint32_t>(conn, Kp * 4);
     d.Dt3 = U.real(dt3, (size_t)3 * Np * Np); d.Lt3 = U.real(lt3, (size_t)4 * Nfp * Np);
+    d.Dfrag = nullptr; d.Lfrag = nullptr;
+    if (s->kern3 == K3_TPG) {
+        // operators in MMA-fragment order, zero-padded, for the kernels that fetch them per use (kernel_vol3d_mmag.cuh /
+        // kernel_vol3d_tf32g.cuh).  fp64: A of mma.m8n8k4, one value per lane.  fp32: B of mma.m16n8k8, per lane the
+        // two k-halves, split into (hi, hi', lo, lo') exactly as split_tf32 does on the device.
+        const bool f64 = std::is_same<T, double>::value;
+        const int MTn = (Np + 7) / 8, kstep = f64 ? 4 : 8, per = f64 ? 1 : 4;
+        const int KDn = (Np + kstep - 1) / kstep, KLn = (Nfp + kstep - 1) / kstep;
+        std::vector<T> df, lf;
+        if (!A.dry) {
+            df.assign((size_t)3 * MTn * KDn * 32 * per, T(0));
+            lf.assign((size_t)4 * MTn * KLn * 32 * per, T(0));
+            auto put = [&](std::vector<T>& out, size_t base, double v0, double v1) {
+                if (f64) { out[base] = (T)v0; return; }
+                const float x[2] = {(float)v0, (float)v1};
+                for (int h = 0; h < 2; ++h) {
+                    uint32_t bits; std::memcpy(&bits, &x[h], 4);
+                    bits &= 0xffffe000u;
+                    float hi; std::memcpy(&hi, &bits, 4);
+                    out[base + h] = (T)hi; out[base + 2 + h] = (T)(x[h] - hi);
+                }
+            };
+            for (int mt = 0; mt < MTn; ++mt)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const int g = lane >> 2, t = lane & 3, n = 8 * mt + g;
+                    if (n >= Np) continue;
+                    for (int a = 0; a < 3; ++a)
+                        for (int sx = 0; sx < KDn; ++sx) {
+                            const int k0 = kstep * sx + t, k1 = k0 + 4;
+                            const double v0 = k0 < Np ? m.r3.D[a][(size_t)n * Np + k0] : 0.0;
+                            const double v1 = (!f64 && k1 < Np) ? m.r3.D[a][(size_t)n * Np + k1] : 0.0;
+                            put(df, ((((size_t)a * MTn + mt) * KDn + sx) * 32 + lane) * per, v0, v1);
+                        }
+                    for (int f = 0; f < 4; ++f)
+                        for (int sx = 0; sx < KLn; ++sx) {
+                            const int j0 = kstep * sx + t, j1 = j0 + 4;
+                            const double v0 = j0 < Nfp ? m.r3.LIFT[(size_t)n * 4 * Nfp + f * Nfp + j0] : 0.0;
+                            const double v1 = (!f64 && j1 < Nfp) ? m.r3.LIFT[(size_t)n * 4 * Nfp + f * Nfp + j1] : 0.0;
+                            put(lf, ((((size_t)f * MTn + mt) * KLn + sx) * 32 + lane) * per, v0, v1);
+                        }
+                }
+        }
+        d.Dfrag = U.real(df, (size_t)3 * MTn * KDn * 32 * per);
+        d.Lfrag = U.real(lf, (size_t)4 * MTn * KLn * 32 * per);
+    }
     d.fmask3 = U.template ints<short>(fm3, 4 * Nfp);
     d.perm3 = U.template ints<uint8_t>(m.perm3, 6 * Nfp);
     // ---- 2D
@@ -802,13 +847,16 @@ int dg_workspace_bytes(const dg_mesh* mesh, int N, int J, int precision, uint64_
         if (!bytes) throw std::runtime_error("EINVAL: NULL argument");
         dg_solver s;
         s.N = N; s.J = J; s.precision = precision;
-        s.kern3 = K3_SCALAR;                                   // upper bound over every dg_options.kernel choice:
-        for (int k = 1; k < K3_COUNT; ++k)                     // a kernel with the extended per-tet record, if one covers (precision, N)
-            if (KERNELS[k].geox && (!KERNELS[k].precision || KERNELS[k].precision == precision) && N >= KERNELS[k].nmin && N <= KERNELS[k].nmax) s.kern3 = k;
         s.m.N = N; s.m.K = mesh->ntets; s.m.C = 8;
         quick_counts(mesh, s.m.T, s.m.E);
         s.m.Np = (N + 1) * (N + 2) * (N + 3) / 6; s.m.Nfp = (N + 1) * (N + 2) / 2; s.m.N1 = N + 1;
-        *bytes = dry_bytes(&s) + 4096;
+        size_t need = 0;                                       // upper bound over every dg_options.kernel choice that
+        for (int k = 1; k < K3_COUNT; ++k) {                   // covers (precision, N): some carry extra per-tet records
+            if ((KERNELS[k].precision && KERNELS[k].precision != precision) || N < KERNELS[k].nmin || N > KERNELS[k].nmax) continue;
+            s.kern3 = k;
+            need = std::max(need, dry_bytes(&s));
+        }
+        *bytes = need + 4096;
         return DG_OK;
     } catch (const std::exception& e) { return err_from_exception(e); }
 }

@@ -1,10 +1,12 @@
 // 3D solver, fp64, tensor-pipe kernel for the degrees whose operator rows do not fit the register file (N >= 6):
 // fused volume + surface + update of one LSRK stage (Alg. 2, eq (41)-(43)).
 // Same mathematics and the same DMMA fragments as kernel_vol3d_mma.cuh (m-tile = 8 nodes, n-tile = 8 elements, k = 4),
-// but the A fragments (rows of D_r, D_s, D_t, LIFT) are fetched per use from the transposed operator arrays, which
-// stay L1/L2-resident (N = 8: 0.9 MB): lane (g,t) reads D[n = 8w+g][m = 4s+t], i.e. four 64-byte row segments per
-// fragment -- the same sectors a dedicated fragment array would cost.  An A fragment feeds NTILE n-tiles
-// (NTILE * 8 elements per batch), which divides the operator traffic per element by NTILE.
+// but the A fragments (rows of D_r, D_s, D_t, LIFT) are fetched per use from global memory, where the host has laid
+// the operators out in FRAGMENT ORDER, zero-padded: Dfrag [3][MT][KD][32], Lfrag [4][MT][KL][32], entry (a, mt, s, lane
+// = 4 g + t) = D_a[n = 8 mt + g][m = 4 s + t].  A fragment is then one unconditional, fully coalesced 256-byte load per
+// warp (two wavefronts; the transposed operator array cost four 64-byte row segments and a bounds check per value),
+// and the arrays stay L1/L2-resident (N = 8: 0.9 MB).  An A fragment feeds NTILE n-tiles (NTILE * 8 elements per
+// batch), which divides the operator traffic per element by NTILE.
 //   phase 1  all threads: (p, contravariant velocity) of every node of the batch -> B operand rows [k][8] per n-tile
 //   phase 2  all threads: one upwind flux jump per face node  -> B operand rows of the LIFT part
 //   phase 3  warp w loops over the m-tiles w, w+W, ...: 6 KD + 4 KL DMMA per n-tile, then the right-hand side and
@@ -98,7 +100,6 @@ k_vol3d_mmag(Dev<double> d, int src, double rka, double rkb, double dt) {
         for (int mt = w; mt < MT; mt += W) {
             const int n = 8 * mt + g;
             const bool nok = n < Np;
-            const int nc = nok ? n : Np - 1;
             double acc[NTILE][10][2];
 #pragma unroll
             for (int q = 0; q < NTILE; ++q)
@@ -106,13 +107,11 @@ k_vol3d_mmag(Dev<double> d, int src, double rka, double rkb, double dt) {
                 for (int v = 0; v < 10; ++v) acc[q][v][0] = acc[q][v][1] = 0.0;
             const double* bp = sB + t * 8 + (g ^ swz(t));
             // operator fragments one k-step ahead: their L1/L2 latency is the cost of this kernel
+            const double* fD = d.Dfrag + (size_t)mt * KD * 32 + lane;
             auto loadD = [&](int s_, double& ar, double& as, double& at) {
-                const int m = 4 * s_ + t;
-                const bool ok = nok && m < Np;
-                const int mc = min(m, Np - 1);
-                ar = ok ? d.Dt3[(0 * Np + mc) * Np + nc] : 0.0;                 // Dt3[a][m][n] = D_a[n][m]
-                as = ok ? d.Dt3[(1 * Np + mc) * Np + nc] : 0.0;
-                at = ok ? d.Dt3[(2 * Np + mc) * Np + nc] : 0.0;
+                ar = fD[s_ * 32];
+                as = fD[(MT * KD + s_) * 32];
+                at = fD[(2 * MT * KD + s_) * 32];
             };
             double ar, as, at;
             loadD(0, ar, as, at);
@@ -133,13 +132,11 @@ k_vol3d_mmag(Dev<double> d, int src, double rka, double rkb, double dt) {
                 }
                 ar = nr; as = ns; at = nt_;
             }
+            const double* fL = d.Lfrag + (size_t)mt * KL * 32 + lane;
             for (int s_ = 0; s_ < KL; ++s_) {
-                const int j = 4 * s_ + t;
-                const bool ok = nok && j < Nfp;
-                const int jc = min(j, Nfp - 1);
 #pragma unroll
                 for (int f = 0; f < 4; ++f) {
-                    const double al = ok ? d.Lt3[(f * Nfp + jc) * Np + nc] : 0.0;   // Lt3[j][n] = LIFT[n][j]
+                    const double al = fL[(f * MT * KL + s_) * 32];
 #pragma unroll
                     for (int q = 0; q < NTILE; ++q)
                         dmma884(acc[q][6 + f], al, bp[q * szT + (4 * KPD + f * KPL + 4 * s_) * 8]);

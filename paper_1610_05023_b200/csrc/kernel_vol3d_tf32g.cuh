@@ -1,7 +1,10 @@
 // 3D solver, fp32, tensor-core kernel for N >= 6: fused volume + surface + update of one LSRK stage (PAPER.md:L623-624,
 // Alg. 2, eq (41)-(43)) with the contractions as error-compensated 3xTF32 (kernel_vol3d_tf32.cuh) and the
 // phase structure of kernel_vol3d_mmag.cuh: the operator fragments (B of mma.m16n8k8: D[n = 8w+g][k = 8s+t, +4]) do
-// not fit the register file at these degrees, so they are read per use through L1/L2 and split hi/lo on the fly.
+// not fit the register file at these degrees, so they are read per use through L1/L2 -- from arrays the host has laid
+// out in FRAGMENT ORDER, zero-padded and already split: Dfrag [3][NTL][KD][32][4], Lfrag [4][NTL][KL][32][4], entry
+// (a, nt, s, lane = 4 g + t) = (hi, hi', lo, lo') of D_a[n = 8 nt + g][k = 8 s + t] and [k + 4]: one unconditional,
+// coalesced 16-byte load per lane replaces two scalar loads, two bounds checks and two splits.
 // A batch is 16 elements (MMA m); warp w loops over the n-tiles (8 nodes) w, w+W, ...
 #pragma once
 #include "kernel_vol3d_tf32.cuh"
@@ -87,9 +90,8 @@ k_vol3d_tf32g(Dev<float> d, int src, float rka, float rkb, float dt) {
         __syncthreads();
         // ---- phase 3: contractions (3xTF32) and update, one n-tile of 8 nodes at a time
         for (int nt = w; nt < NTL; nt += W) {
-            const int nb0 = 8 * nt + g;                      // B-fragment column (node) of this lane
-            const bool bok = nb0 < Np;
-            const int nbc = bok ? nb0 : Np - 1;
+            const uint4* fD = reinterpret_cast<const uint4*>(d.Dfrag) + (size_t)nt * KD * 32 + lane;
+            const uint4* fL = reinterpret_cast<const uint4*>(d.Lfrag) + (size_t)nt * KL * 32 + lane;
             float cpr[4] = {0, 0, 0, 0}, cps[4] = {0, 0, 0, 0}, cpt[4] = {0, 0, 0, 0};
             float cvr[4] = {0, 0, 0, 0}, cvs[4] = {0, 0, 0, 0}, cvt[4] = {0, 0, 0, 0};
             float cl[4][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
@@ -104,14 +106,11 @@ k_vol3d_tf32g(Dev<float> d, int src, float rka, float rkb, float dt) {
 #pragma unroll 1
             for (int s_ = 0; s_ < KD; ++s_) {
                 uint32_t brh[2], brl[2], bsh[2], bsl[2], bth[2], btl[2];
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int m = 8 * s_ + t + 4 * h;
-                    const bool ok = bok && m < Np;
-                    const int mc = min(m, Np - 1);
-                    split_tf32(ok ? d.Dt3[(0 * Np + mc) * Np + nbc] : 0.f, brh[h], brl[h]);    // Dt3[a][m][n] = D_a[n][m]
-                    split_tf32(ok ? d.Dt3[(1 * Np + mc) * Np + nbc] : 0.f, bsh[h], bsl[h]);
-                    split_tf32(ok ? d.Dt3[(2 * Np + mc) * Np + nbc] : 0.f, bth[h], btl[h]);
+                {
+                    const uint4 vr = fD[s_ * 32], vs = fD[(NTL * KD + s_) * 32], vt = fD[(2 * NTL * KD + s_) * 32];
+                    brh[0] = vr.x; brh[1] = vr.y; brl[0] = vr.z; brl[1] = vr.w;
+                    bsh[0] = vs.x; bsh[1] = vs.y; bsl[0] = vs.z; bsl[1] = vs.w;
+                    bth[0] = vt.x; bth[1] = vt.y; btl[0] = vt.z; btl[1] = vt.w;
                 }
                 uint32_t ph[4], pl[4], rh[4], rl[4], sh[4], sl[4], th[4], tl[4];
                 loadA(ap + (8 * s_) * XS, ph, pl);
@@ -131,11 +130,9 @@ k_vol3d_tf32g(Dev<float> d, int src, float rka, float rkb, float dt) {
 #pragma unroll
                 for (int f = 0; f < 4; ++f) {
                     uint32_t bh[2], bl[2], ah[4], al[4];
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const int j = 8 * s_ + t + 4 * h;
-                        const bool ok = bok && j < Nfp;
-                        split_tf32(ok ? d.Lt3[(f * Nfp + min(j, Nfp - 1)) * Np + nbc] : 0.f, bh[h], bl[h]);   // Lt3[j][n] = LIFT[n][j]
+                    {
+                        const uint4 v = fL[(f * NTL * KL + s_) * 32];
+                        bh[0] = v.x; bh[1] = v.y; bl[0] = v.z; bl[1] = v.w;
                     }
                     loadA(gp + (f * KPL + 8 * s_) * XS, ah, al);
                     mma_3x(cl[f], ah, al, bh, bl);

@@ -32,6 +32,8 @@ struct Dev {
     const uint32_t* conn3;           // [K][4]  packed (kernel_vol3d_mma.cuh): boundary flag | id << 5 | perm << 2 | face
     const T* Dt3;                    // [3][Np][Np]  Dt3[a][m][n] = D_a[n][m]
     const T* Lt3;                    // [4 Nfp][Np]  Lt3[j][n]   = LIFT[n][j]
+    const T* Dfrag; const T* Lfrag;  // the same operators in MMA-fragment order, zero-padded (N >= 6 tensor-pipe kernels
+                                     // only; layouts in kernel_vol3d_mmag.cuh / kernel_vol3d_tf32g.cuh), else NULL
     const short* fmask3;             // [4][Nfp]
     const uint8_t* perm3;            // [6][Nfp]
     // ---- 2D

@@ -67,6 +67,16 @@ def test_J8_degree(N):
         _check(parity.compare(lib, ora), prec)
 
 
+@pytest.mark.parametrize("N,J", [(2, 1), (3, 3), (5, 5), (4, 7), (5, 6), (3, 9)])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_partial_set_groups(N, J, prec):
+    """The 2D solvers work on groups of four auxiliary sets: J that is not a multiple of four leaves a partial last
+    group (1, 2 or 3 sets), J > 8 three groups per triangle.  fp64 runs k_face2d_mma, fp32 k_face2d."""
+    w = make_workload("cfg3", n=3, N=N, J=J, nsteps=15)
+    lib, ora = parity.run_library(w, precision=prec), parity.run_oracle(w)
+    _check(parity.compare(lib, ora), prec)
+
+
 @pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (5, 1), (5, 2), (5, 3), (1, 2), (2, 2), (6, 1), (6, 5), (7, 1), (7, 5), (8, 5)])
 def test_3d_kernel_variants(N, kernel):
     """dg_options.kernel (DG_KERNEL_*): 1 scalar FMA, 2 batch-synchronous DMMA, 3 warp-specialised DMMA, 5 tensor pipe
