@@ -27,7 +27,7 @@ template <int N>
 __global__ void __launch_bounds__(ElemCfg<N>::NT) k_vol3d_elem(Dev<float> d, int src, float rka, float rkb, float dt) {
     using C = ElemCfg<N>;
     constexpr int Np = C::Np, Nfp = C::Nfp, Nfn = C::Nfn, NT = C::NT;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     float* sX = reinterpret_cast<float*>(smem_raw);          // [4][Np][NT]: p, U^r, U^s, U^t of this thread's element
     int* sNb = reinterpret_cast<int*>(sX + 4 * Np * NT);     // [24][Nfp]: (neighbour face | perm << 2, j) -> neighbour node
     int* sFm = sNb + 24 * Nfp;                               // [4][Nfp] own face node
