@@ -74,6 +74,9 @@ typedef struct {
                                  end of the axis): 0 = HABC (the default), 1 = p = 0 (free surface),
                                  2 = rigid wall (n.u = 0).  Auxiliary fields exist only on HABC faces, on the edges
                                  between two of them and at the corners where three meet */
+    int32_t time_kernels;     /* 1: every step also records a CUDA event before and after the 3D kernel of each of its five
+                                 stages, on the solver's stream and inside the replayed graph (no host synchronisation, no
+                                 change to the kernels); read them with dg_last_step_kernel_ms.  0 (default): no events */
 } dg_options;
 
 typedef struct {
@@ -145,6 +148,12 @@ int dg_mesh_counts(const dg_mesh* mesh, const int32_t* face_bc, int32_t* counts)
  * with CUDA events around every launch; for per-kernel reporting, never inside a timed benchmark region).
  * ms[0..5] = volume+surface+update 3D, 2D update, 1D update, face closure, edge closure, corner closure. */
 int dg_profile_step(dg_solver* s, double* ms);
+
+/* Device time of the 3D kernel in each of the five LSRK stages of the LAST step that dg_step enqueued, from the events
+ * of dg_options.time_kernels = 1 (DG_EINVAL without it or before the first step).  Unlike dg_profile_step this measures
+ * the kernels where they really run: inside the timed region of a benchmark, back to back with the other kernels, in
+ * the CUDA graph.  Synchronises the stream.  ms: [5], host. */
+int dg_last_step_kernel_ms(dg_solver* s, double* ms);
 
 /* Raw device pointers of the current state, in the library's own layout (optional, lets a caller read
  * traces or fields on the device without the fp64 host round trip of dg_get_fields).  The pointers stay owned by the

@@ -24,7 +24,7 @@ class _Mesh(C.Structure):
 class _Options(C.Structure):
     _fields_ = [("precision", C.c_int32), ("cfl", C.c_double), ("dt", C.c_double), ("stream", C.c_void_p),
                 ("device", C.c_int32), ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64),
-                ("use_graph", C.c_int32), ("kernel", C.c_int32), ("face_bc", C.c_int32 * 6)]
+                ("use_graph", C.c_int32), ("kernel", C.c_int32), ("face_bc", C.c_int32 * 6), ("time_kernels", C.c_int32)]
 
 
 class _Info(C.Structure):
@@ -41,7 +41,7 @@ class _DeviceView(C.Structure):
 
 EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_set_source", "dg_step",
            "dg_get_fields", "dg_get_face_map", "dg_get_edge_map", "dg_reference_element", "dg_mesh_counts",
-           "dg_profile_step", "dg_get_device_ptrs", "dg_last_error", "dg_destroy"]
+           "dg_profile_step", "dg_last_step_kernel_ms", "dg_get_device_ptrs", "dg_last_error", "dg_destroy"]
 
 
 def lib() -> C.CDLL:
@@ -115,7 +115,7 @@ class Solver:
 
     def __init__(self, verts, tets, N: int, J: int, c, rho, precision: int = 64, cfl: float = 1.0,
                  dt: float = 0.0, device: int = 0, use_graph: bool = True, torch_workspace: bool = True,
-                 kernel: int = 0, face_bc=None):
+                 kernel: int = 0, face_bc=None, time_kernels: bool = False):
         """face_bc: None (HABC everywhere) or {(axis, sign): "habc" | "dirichlet" | "rigid"} for some of the six domain
         faces (axis 0..2, sign -1/+1) -- dg_options.face_bc."""
         import torch                                          # device memory + stream only
@@ -128,6 +128,7 @@ class Solver:
         opt = _Options()
         opt.precision, opt.cfl, opt.dt, opt.device, opt.use_graph = precision, cfl, dt, device, int(use_graph)
         opt.kernel = int(kernel)
+        opt.time_kernels = int(time_kernels)
         for i, code in enumerate(_face_bc_codes(face_bc)):
             opt.face_bc[i] = int(code)
         self._torch = torch
@@ -212,6 +213,13 @@ class Solver:
         xyz = np.empty((self.E, self.N + 1, 3))
         _check(lib().dg_get_edge_map(self._h, _ip(axis), _ip(nax), _ip(sg), _dp(xyz)))
         return axis, nax, sg, xyz
+
+    def last_step_kernel_ms(self):
+        """dg_last_step_kernel_ms: device time of the 3D kernel in the five stages of the last step, from events recorded
+        inside the step itself (Solver(..., time_kernels=True))."""
+        ms = np.zeros(5)
+        _check(lib().dg_last_step_kernel_ms(self._h, _dp(ms)))
+        return ms
 
     def profile_step(self):
         ms = np.zeros(6)

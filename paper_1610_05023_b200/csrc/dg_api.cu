@@ -95,6 +95,9 @@ struct dg_solver {
     double* t_dev = nullptr;        // simulated time at the start of the current step (advanced by k_source while a source is on)
     double t_host = 0;              // the same clock kept on the host (dg_step adds dt per step), so that a source
                                     // switched on after some steps starts at the right time
+    bool time_kernels = false;      // dg_options.time_kernels: events around the 3D kernel of every stage
+    cudaEvent_t evk[2][5][2] = {};  // [parity of the step's first buffer][stage][before, after]
+    int last_par = -1;              // parity of the last enqueued step (-1: none yet)
     double* export_buf = nullptr;   // device scratch for dg_get_fields (aux fields, fp64)
     size_t export_elems = 0;
 };
@@ -603,9 +606,19 @@ void launch_source(dg_solver* s, Dev<T>& d, int src, int stage) {
 }
 
 template <typename T>
-void launch_stage(dg_solver* s, Dev<T>& d, int src, int stage) {
+void launch_stage(dg_solver* s, Dev<T>& d, int src, int stage, int par) {
     const double a = RKA[stage], b = RKB[stage];
+    // inside a stream capture an event only becomes a real record node of the graph with cudaEventRecordExternal
+    // (the flag is invalid outside a capture)
+    unsigned evflag = cudaEventRecordDefault;
+    if (s->time_kernels) {
+        cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+        cu(cudaStreamIsCapturing(s->stream, &st), "capture status");
+        if (st == cudaStreamCaptureStatusActive) evflag = cudaEventRecordExternal;
+        cu(cudaEventRecordWithFlags(s->evk[par][stage][0], s->stream, evflag), "event record");
+    }
     launch_vol3d<T>(s, d, src, a, b, false);
+    if (s->time_kernels) cu(cudaEventRecordWithFlags(s->evk[par][stage][1], s->stream, evflag), "event record");
     launch_source<T>(s, d, src, stage);
     if (d.J > 0 && d.Tn > 0) {
         launch_face2d<T>(s, d, src, a, b);
@@ -630,8 +643,9 @@ int launches_per_stage(const dg_solver* s) {
 
 template <typename T>
 void run_step_plain(dg_solver* s, Dev<T>& d) {
+    const int par = s->cur;
     for (int st = 0; st < 5; ++st) {
-        launch_stage<T>(s, d, s->cur, st);
+        launch_stage<T>(s, d, s->cur, st, par);
         s->cur ^= 1;
     }
 }
@@ -639,7 +653,7 @@ void run_step_plain(dg_solver* s, Dev<T>& d) {
 template <typename T>
 void run_steps(dg_solver* s, Dev<T>& d, int nsteps) {
     if (!s->use_graph) {
-        for (int i = 0; i < nsteps; ++i) run_step_plain<T>(s, d);
+        for (int i = 0; i < nsteps; ++i) { s->last_par = s->cur; run_step_plain<T>(s, d); }
         cu(cudaGetLastError(), "kernel launch");
         return;
     }
@@ -665,6 +679,7 @@ void run_steps(dg_solver* s, Dev<T>& d, int nsteps) {
             cu(e, "graph instantiate");
         }
         cu(cudaGraphLaunch(s->graph[par], s->stream), "graph launch");
+        s->last_par = par;
         s->cur = par ^ 1;              // five stages flip the parity once
     }
 }
@@ -876,6 +891,7 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         s->stream = opt ? (cudaStream_t)opt->stream : nullptr;
         s->use_graph = opt ? opt->use_graph != 0 : true;
         s->kern3 = resolve_kernel(opt ? opt->kernel : 0, precision, N);
+        s->time_kernels = opt && opt->time_kernels != 0;
         if (mesh->ntets > CONN_MAX_ID) throw std::runtime_error("EINVAL: more than 2^26 - 1 tetrahedra");
         if (!s->stream) s->use_graph = false;      // the legacy default stream cannot be captured
         s->rho.assign(rho, rho + mesh->ntets);
@@ -892,6 +908,8 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
         const double cfl = (opt && opt->cfl > 0) ? opt->cfl : 1.0;
         s->dt = (opt && opt->dt > 0) ? opt->dt : cfl * dtmin;
         cu(cudaSetDevice(s->device), "cudaSetDevice");
+        if (s->time_kernels)
+            for (auto& par : s->evk) for (auto& st : par) for (auto& e : st) cu(cudaEventCreate(&e), "event create");
         const size_t need = dry_bytes(s);
         if (opt && opt->workspace_dev) {
             if (opt->workspace_bytes < need) throw std::runtime_error("ENOMEM: workspace_bytes is smaller than dg_workspace_bytes");
@@ -928,6 +946,7 @@ void dg_destroy(dg_solver* s) {
     cudaSetDevice(s->device);
     cudaStreamSynchronize(s->stream);      // dg_step is asynchronous: nothing may still be writing the workspace
     for (int i = 0; i < 2; ++i) if (s->graph[i]) cudaGraphExecDestroy(s->graph[i]);
+    for (auto& par : s->evk) for (auto& st : par) for (auto& e : st) if (e) cudaEventDestroy(e);
     if (s->own_ws && s->ws) cudaFree(s->ws);
     delete s;
 }
@@ -1089,6 +1108,22 @@ int dg_get_edge_map(const dg_solver* s, int32_t* axis, int32_t* normal_axes, int
                 }
     }
     return DG_OK;
+}
+
+int dg_last_step_kernel_ms(dg_solver* s, double* ms) {
+    try {
+        if (!s || !ms) throw std::runtime_error("EINVAL: NULL argument");
+        if (!s->time_kernels) throw std::runtime_error("EINVAL: the solver was created without dg_options.time_kernels");
+        if (s->last_par < 0) throw std::runtime_error("EINVAL: no step has been enqueued yet");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        cu(cudaStreamSynchronize(s->stream), "sync");
+        for (int st = 0; st < 5; ++st) {
+            float t = 0;
+            cu(cudaEventElapsedTime(&t, s->evk[s->last_par][st][0], s->evk[s->last_par][st][1]), "elapsed");
+            ms[st] = t;
+        }
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
 }
 
 int dg_get_device_ptrs(const dg_solver* s, dg_device_view* o) {

@@ -260,6 +260,38 @@ def test_device_view_matches_get_fields(prec):
     s.close()
 
 
+def test_in_step_kernel_timing():
+    """dg_options.time_kernels: events inside the (graph-replayed) step give the 3D kernel's time per stage; the numbers
+    are positive, below the whole step's time, and the option does not change the result."""
+    import time
+    import torch
+    from paper_1610_05023_b200 import DgError, Solver
+    w = make_workload("cfg5", n=6, nsteps=5)
+    out = []
+    for timed in (False, True):
+        s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, time_kernels=timed)
+        x, y, z = s.get_nodes()
+        s.set_initial(*parity.initial_on(w, x, y, z, w.c, w.rho))
+        if timed:
+            with pytest.raises(DgError):
+                s.last_step_kernel_ms()                      # no step yet
+        s.step(4)
+        s.stream.synchronize()
+        t0 = time.perf_counter()
+        s.step(1)
+        s.stream.synchronize()
+        step_ms = 1e3 * (time.perf_counter() - t0)
+        if timed:
+            ms = s.last_step_kernel_ms()
+            assert ms.shape == (5,) and (ms > 0).all() and ms.sum() < step_ms, (ms, step_ms)
+        else:
+            with pytest.raises(DgError):
+                s.last_step_kernel_ms()
+        out.append(s.get_fields()[0])
+        s.close()
+    assert np.array_equal(out[0], out[1])
+
+
 def test_missing_device_is_loud(monkeypatch):
     import torch
     from paper_1610_05023_b200 import DgError, Solver
