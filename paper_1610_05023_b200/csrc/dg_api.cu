@@ -452,7 +452,7 @@ void vol3d_ws(dg_solver* s, Dev<double>& d, int src, double a, double b, bool cf
 template <int N>
 void vol3d_tf32(dg_solver* s, Dev<float>& d, int src, double a, double b, bool cfg) {
     using Cfg = TfCfg<N>;
-    run_vol3d(s, k_vol3d_tf32<N>, Cfg::NT, Cfg::smem_bytes, Cfg::EB, d.K, true, cfg, d, (const float*)s->geox3, src, (float)a, (float)b);
+    run_vol3d(s, k_vol3d_tf32<N>, Cfg::NT, Cfg::smem_bytes, Cfg::EB, d.K, Cfg::MINB == 1, cfg, d, (const float*)s->geox3, src, (float)a, (float)b);
 }
 template <int N>
 void vol3d_mmag(dg_solver* s, Dev<double>& d, int src, double a, double b, bool cfg) {

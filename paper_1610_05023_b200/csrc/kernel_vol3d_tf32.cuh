@@ -35,7 +35,10 @@ struct TfCfg {
     static constexpr int KD = (Np + 7) / 8, KPD = KD * 8;
     static constexpr int KL = (Nfp + 7) / 8, KPL = KL * 8;
     static constexpr int XS = 24;                      // operand row stride in floats (16 elements + 8: bank spread)
-    static constexpr int NT = 384;
+    // warp roles: MMA warps 0..MT-1, LOADER warp LW, PREP warps PW0..PW0+3.  With MT <= 3 (N = 3) the roles fit two
+    // warpgroups and two CTAs share an SM (six MMA warps per SM instead of three); otherwise three warpgroups, one CTA
+    static constexpr bool COMPACT = MT <= 3;
+    static constexpr int NT = COMPACT ? 256 : 384, LW = COMPACT ? 3 : 7, PW0 = COMPACT ? 4 : 8, MINB = COMPACT ? 2 : 1;
     static constexpr int NS = 3;                       // staging depth
     static constexpr int QS = Np * 4 + 4;              // staged element stride of q / res in floats (16 B skew)
     static constexpr int GS = GX3 + 8;                 // staged stride of the record (208 B = 13 x 16 B: bank spread)
@@ -51,8 +54,11 @@ struct TfCfg {
     static constexpr uint32_t tx_bytes = 2 * EB * Np * 16 + EB * GX3 * 4;
     static constexpr int NRA = (Np + 1) / 2;           // PREP phase A rows: 2 nodes x 16 elements
     static constexpr int NRB = 2 * Nfp;                // PREP phase B rows: (face node j, face pair) x 2 faces x 16 elements
-    static constexpr int REG_BASE = 168, REG_PREP = 88, REG_MMA = 208;
-    static_assert((REG_BASE - REG_PREP) * 128 >= (REG_MMA - REG_BASE) * 256, "setmaxnreg pool would deadlock");
+    // setmaxnreg: launched with REG_BASE registers per thread (65536 / (NT * MINB)); what the PREP warpgroup gives back
+    // is the only pool the MMA warpgroup(s) can grow from
+    static constexpr int REG_BASE = COMPACT ? 128 : 168, REG_PREP = 88, REG_MMA = COMPACT ? 168 : 208;
+    static_assert((REG_BASE - REG_PREP) * 128 >= (REG_MMA - REG_BASE) * (NT - 128), "setmaxnreg pool would deadlock");
+    static_assert(REG_BASE * NT * MINB <= 65536, "register file");
     static_assert(MT <= 7, "the tensor-core fp32 kernel covers N <= 5");
     static_assert(smem_bytes <= 227 * 1024, "shared memory");
 };
@@ -76,7 +82,7 @@ __device__ __forceinline__ void mma_3x(float (&c)[4], const uint32_t (&ah)[4], c
 }
 
 template <int N>
-__global__ void __launch_bounds__(TfCfg<N>::NT, 1)
+__global__ void __launch_bounds__(TfCfg<N>::NT, TfCfg<N>::MINB)
 k_vol3d_tf32(Dev<float> d, const float* __restrict__ geox, int src, float rka, float rkb) {
     using C = TfCfg<N>;
     constexpr int Np = C::Np, Nfp = C::Nfp, Nfn = C::Nfn, EB = C::EB, KD = C::KD, KPD = C::KPD, KL = C::KL, KPL = C::KPL,
@@ -114,10 +120,10 @@ k_vol3d_tf32(Dev<float> d, const float* __restrict__ geox, int src, float rka, f
     }
     __syncthreads();
 
-    if (w >= 8) {
+    if (w >= C::PW0) {
         // =============================================================== PREP warps
         reg_dec<C::REG_PREP>();
-        const int pw = w - 8;
+        const int pw = w - C::PW0;
         const int ie = lane & 15, fh = lane >> 4;
         int it = 0;
         for (int b = blockIdx.x; b < nbatch; b += gridDim.x, ++it) {
@@ -166,7 +172,7 @@ k_vol3d_tf32(Dev<float> d, const float* __restrict__ geox, int src, float rka, f
     }
 
     reg_inc<C::REG_MMA>();
-    if (w == 7) {
+    if (w == C::LW) {
         // =============================================================== LOADER warp
         // half-warp hw gathers faces 2 hw and 2 hw + 1 of element ie: one 16-byte cp.async per face node (p,u,v,w)
         const int ie = lane & 15, hw = lane >> 4;
