@@ -38,11 +38,11 @@ typedef struct dg_solver dg_solver; /* opaque, owned by the library; free with d
 
 /* dg_options.kernel: which kernel runs the fused 3D volume + surface + update stage (eq (41)-(43)).
  * All of them compute the same stage; they differ in how the D_r/D_s/D_t and LIFT contractions are carried out. */
-#define DG_KERNEL_AUTO 0   /* fp64: MMA for N <= 4, WS at N = 5, TPG for N >= 6; fp32: ELEM for N <= 2, TF32 for
+#define DG_KERNEL_AUTO 0   /* fp64: MMA for N = 1, 2, 4, WS at N = 3, 5, TPG for N >= 6; fp32: ELEM for N <= 2, TF32 for
                               N = 3..5, TPG for N >= 6 */
 #define DG_KERNEL_SCALAR 1 /* scalar FMA, operators in shared memory (or L1/L2 for high N); fp64 and fp32, N = 1..8 */
 #define DG_KERNEL_MMA 2    /* fp64 DMMA (mma.sync.m8n8k4.f64), operator rows register-resident; N = 1..5 */
-#define DG_KERNEL_WS 3     /* DG_KERNEL_MMA with warp-specialised loader / operand / MMA roles; fp64, N = 4, 5 */
+#define DG_KERNEL_WS 3     /* DG_KERNEL_MMA with warp-specialised loader / operand / MMA roles; fp64, N = 1..5 */
 #define DG_KERNEL_TF32 4   /* fp32 on the tensor cores as error-compensated 3xTF32 (fp32-accurate); N = 3..5 */
 #define DG_KERNEL_TPG 5    /* tensor-pipe kernels for the degrees whose operators do not fit the register file:
                               fp64 DMMA / fp32 3xTF32; N = 6..8 */

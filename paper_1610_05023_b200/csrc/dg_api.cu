@@ -115,13 +115,13 @@ const KernRow KERNELS[K3_COUNT] = {
     {0, 1, 8, false, "auto"},
     {0, 1, 8, false, "scalar-FMA kernel (kernel = 1): fp64/fp32, N = 1..8"},
     {64, 1, 5, false, "fp64 tensor-pipe kernel (kernel = 2): fp64, N = 1..5"},
-    {64, 4, 5, true, "warp-specialised fp64 tensor-pipe kernel (kernel = 3): fp64, N = 4, 5"},
+    {64, 1, 5, true, "warp-specialised fp64 tensor-pipe kernel (kernel = 3): fp64, N = 1..5"},
     {32, 3, 5, true, "fp32 3xTF32 tensor-core kernel (kernel = 4): fp32, N = 3..5"},
     {0, 6, 8, false, "tensor-pipe kernels with operators read through L1/L2 (kernel = 5): N = 6..8"},
     {32, 1, 2, false, "thread-per-element fp32 kernel (kernel = 6): fp32, N = 1, 2"},
 };
 //                                    N =      1          2          3        4        5      6       7       8
-const int DEFAULT_KERNEL_F64[9] = {0, K3_MMA,    K3_MMA,    K3_MMA,  K3_MMA,  K3_WS,   K3_TPG, K3_TPG, K3_TPG};
+const int DEFAULT_KERNEL_F64[9] = {0, K3_MMA,    K3_MMA,    K3_WS,   K3_MMA,  K3_WS,   K3_TPG, K3_TPG, K3_TPG};
 const int DEFAULT_KERNEL_F32[9] = {0, K3_ELEM,   K3_ELEM,   K3_TF32, K3_TF32, K3_TF32, K3_TPG, K3_TPG, K3_TPG};
 
 int resolve_kernel(int requested, int precision, int N) {
@@ -447,7 +447,7 @@ void vol3d_mma(dg_solver* s, Dev<double>& d, int src, double a, double b, bool c
 template <int N>
 void vol3d_ws(dg_solver* s, Dev<double>& d, int src, double a, double b, bool cfg) {
     using Cfg = WsCfg<N>;
-    run_vol3d(s, k_vol3d_ws<N>, Cfg::NT, Cfg::smem_bytes, Cfg::EB, d.K, true, cfg, d, (const double*)s->geox3, src, a, b);
+    run_vol3d(s, k_vol3d_ws<N>, Cfg::NT, Cfg::smem_bytes, Cfg::EB, d.K, Cfg::MINB == 1, cfg, d, (const double*)s->geox3, src, a, b);
 }
 template <int N>
 void vol3d_tf32(dg_solver* s, Dev<float>& d, int src, double a, double b, bool cfg) {
@@ -510,7 +510,9 @@ void launch_vol3d(dg_solver* s, Dev<T>& d, int src, double a, double b, bool cfg
             break;
         case K3_WS:
             if constexpr (F64) switch (N) {
-                DG_CASE(4, vol3d_ws<4>(s, d, src, a, b, cfg)); DG_CASE(5, vol3d_ws<5>(s, d, src, a, b, cfg));
+                DG_CASE(1, vol3d_ws<1>(s, d, src, a, b, cfg)); DG_CASE(2, vol3d_ws<2>(s, d, src, a, b, cfg));
+                DG_CASE(3, vol3d_ws<3>(s, d, src, a, b, cfg)); DG_CASE(4, vol3d_ws<4>(s, d, src, a, b, cfg));
+                DG_CASE(5, vol3d_ws<5>(s, d, src, a, b, cfg));
             }
             break;
         case K3_TF32:

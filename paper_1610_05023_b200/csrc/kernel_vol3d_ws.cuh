@@ -36,7 +36,10 @@ struct WsCfg {
     static constexpr int KD = (Np + 3) / 4, KPD = KD * 4;
     static constexpr int KL = (Nfp + 3) / 4, KPL = KL * 4;
     static constexpr int LPAD = KPL * EB + 8;          // stride of one face block of the flux operand (bank spread)
-    static constexpr int NT = 384;
+    // warp roles: MMA warps 0..MT-1, LOADER warp LW, PREP warps PW0..PW0+3.  With MT <= 3 (N <= 3) the roles fit two
+    // warpgroups and two CTAs share an SM; otherwise three warpgroups, one CTA per SM
+    static constexpr bool COMPACT = MT <= 3;
+    static constexpr int NT = COMPACT ? 256 : 384, LW = COMPACT ? 3 : 7, PW0 = COMPACT ? 4 : 8, MINB = COMPACT ? 2 : 1;
     static constexpr int NS = 3;                       // staging depth
     // staged q / res: element e sits at e * QS + 2 * slot(e) doubles, QS a multiple of 128 bytes and slot(e) a
     // permutation of the eight 16-byte bank groups chosen so that BOTH access patterns are conflict-free: PREP
@@ -59,8 +62,9 @@ struct WsCfg {
     static constexpr int PITEM = (Nfn + 3) / 4;        // face nodes per LOADER lane
     // setmaxnreg: the kernel is compiled for 168 registers (65536 / 384 rounded down to a multiple of 8); the
     // registers the PREP warpgroup gives back are the only pool the two MMA warpgroups can grow from
-    static constexpr int REG_BASE = 168, REG_PREP = 88, REG_MMA = 208;
-    static_assert((REG_BASE - REG_PREP) * 128 >= (REG_MMA - REG_BASE) * 256, "setmaxnreg pool would deadlock");
+    static constexpr int REG_BASE = COMPACT ? 128 : 168, REG_PREP = 88, REG_MMA = COMPACT ? 168 : 208;
+    static_assert((REG_BASE - REG_PREP) * 128 >= (REG_MMA - REG_BASE) * (NT - 128), "setmaxnreg pool would deadlock");
+    static_assert(REG_BASE * NT * MINB <= 65536, "register file");
     static_assert(MT <= 7, "the warp-specialised kernel covers N <= 5");
 };
 
@@ -86,7 +90,7 @@ __device__ __forceinline__ void bar_sync64(int id) { asm volatile("bar.sync %0, 
 __device__ __forceinline__ void bar_arrive64(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
 
 template <int N>
-__global__ void __launch_bounds__(WsCfg<N>::NT, 1)
+__global__ void __launch_bounds__(WsCfg<N>::NT, WsCfg<N>::MINB)
 k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, double rkb) {
     using C = WsCfg<N>;
     constexpr int Np = C::Np, Nfp = C::Nfp, Nfn = C::Nfn, EB = C::EB, KD = C::KD, KPD = C::KPD, KL = C::KL,
@@ -124,10 +128,10 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
     }
     __syncthreads();
 
-    if (w >= 8) {
+    if (w >= C::PW0) {
         // =============================================================== PREP warps
         reg_dec<C::REG_PREP>();
-        const int pw = w - 8;
+        const int pw = w - C::PW0;
         const int ie = lane & 7, f = lane >> 3;
         const int slot = f + 4 * pw;                         // phase A: nodes slot + 16 r of element ie
         int fmo[NJ];                                         // phase B: own node of face node j = pw + 4 r of face f
@@ -189,7 +193,7 @@ k_vol3d_ws(Dev<double> d, const double* __restrict__ geox, int src, double rka, 
     }
 
     reg_inc<C::REG_MMA>();
-    if (w == 7) {
+    if (w == C::LW) {
         // =============================================================== LOADER warp
         // gather role: lanes 2k, 2k+1 fetch the two 16-byte halves of one node's (p,u,v,w): one 32-byte sector
         const int ie = (lane >> 1) & 7, h = lane & 1, hw = lane >> 4;

@@ -77,7 +77,7 @@ def test_partial_set_groups(N, J, prec):
     _check(parity.compare(lib, ora), prec)
 
 
-@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (5, 1), (5, 2), (5, 3), (1, 2), (2, 2), (6, 1), (6, 5), (7, 1), (7, 5), (8, 5)])
+@pytest.mark.parametrize("N,kernel", [(4, 1), (4, 2), (4, 3), (5, 1), (5, 2), (5, 3), (1, 2), (2, 2), (1, 3), (2, 3), (3, 3), (3, 2), (6, 1), (6, 5), (7, 1), (7, 5), (8, 5)])
 def test_3d_kernel_variants(N, kernel):
     """dg_options.kernel (DG_KERNEL_*): 1 scalar FMA, 2 batch-synchronous DMMA, 3 warp-specialised DMMA, 5 tensor pipe
     with the operators read through L1/L2 (N >= 6) -- the same numbers.
@@ -106,7 +106,7 @@ def test_kernel_choice_is_validated():
     """a kernel that does not cover (precision, N) is refused with DG_EINVAL, not silently replaced"""
     from paper_1610_05023_b200 import DgError, Solver
     w = make_workload("cfg1")
-    for N, prec, kernel in ((6, 64, 2), (3, 64, 3), (5, 64, 4), (2, 32, 4), (5, 32, 5), (3, 32, 6), (2, 64, 6), (3, 64, 7), (3, 64, -1)):
+    for N, prec, kernel in ((6, 64, 2), (6, 64, 3), (5, 64, 4), (2, 32, 4), (5, 32, 5), (3, 32, 6), (2, 64, 6), (3, 64, 7), (3, 64, -1)):
         with pytest.raises(DgError):
             Solver(w.verts, w.tets, N, 2, w.c, w.rho, precision=prec, kernel=kernel)
 
