@@ -21,7 +21,9 @@
 // the fly.  The accumulator fragment of lane (g,t) holds elements g, g+8 x nodes 8w+2t, 8w+2t+1 of all eight
 // results (d_r p, d_s p, d_t p, div U, LIFT_f g), so the update stage runs in registers; it uses the FMA pipe and
 // does not compete with the tensor pipe.  Warp roles, staging, barriers and the per-tet record are those of
-// kernel_vol3d_ws.cuh (LOADER: cp.async.bulk + cp.async gathers; PREP: operands and flux jumps; MMA + update).
+// kernel_vol3d_ws.cuh (LOADER: cp.async.bulk + cp.async gathers; PREP: operands and flux jumps; MMA + update), including
+// the compact two-warpgroup layout with two CTAs per SM at N = 3 (TfCfg::COMPACT: 816 -> 509 us per launch on the
+// SEAM-shaped workload).
 #pragma once
 #include "kernel_vol3d_ws.cuh"
 

@@ -13,6 +13,9 @@
 //                           into stage s of NS, all completing on full[s]
 //   warps 8..11    PREP     wait full[s]; build the operands (p, contravariant velocity; one upwind flux jump per
 //                           face node) into operand buffer o; signal ready[o]
+// With at most three m-tiles (N <= 3) the same roles are packed into two warpgroups -- MMA 0..MT-1, LOADER 3, PREP
+// 4..7, 256 threads -- and two CTAs share an SM (WsCfg::COMPACT): in the 12-warp layout four warps would only hold
+// registers and an SM would run three MMA warps (N = 3 on the SEAM-shaped workload: 1075 -> 753 us per launch).
 // PREP runs one batch ahead of MMA, LOADER up to NS-1 batches ahead.  Register budget (setmaxnreg): the two
 // MMA warpgroups take 208 registers per thread (132 of them hold the operator fragments), PREP 88.
 #pragma once
