@@ -172,6 +172,41 @@ typedef struct {
 } dg_device_view;
 int dg_get_device_ptrs(const dg_solver* s, dg_device_view* out);
 
+/* dg_get_aux_fields_noalloc — the auxiliary-field read-back of dg_get_fields for callers that must not allocate.
+ *
+ * Who needs it.  dg_get_fields converts the face / edge auxiliary state to the physical fields p_i00 (eq (29),
+ * PAPER.md:L384) and p_ij0 (eq (32)) in a device staging buffer before copying it to the host.  That staging
+ * buffer is part of the solver's workspace, which somebody had to allocate: dg_create with cudaMalloc, or the caller
+ * with its own allocator.  Some hosts can do neither at the moment they want the data: a process whose device memory
+ * is handed out in full to another owner at start-up (a framework's caching pool, a fixed partition per tenant) and
+ * has no allocator left to ask; a monitoring or checkpoint thread that runs while another thread of the process is in
+ * a global-mode stream capture, during which cudaMalloc is an error; a time-critical loop that cannot take the
+ * device-wide synchronisation cudaMalloc / cudaFree imply.  This call stages through a fixed array that lives inside
+ * libdg_habc.so itself instead, so it asks nobody for memory.
+ *
+ * What it does.  Same result, bit for bit, as dg_get_fields(s, NULL, NULL, NULL, NULL, face_aux, edge_aux): face_aux
+ * [T][J][3][Nfp], edge_aux [E][J*J][2][N+1], HOST buffers owned by the caller, either may be NULL.  The input is the
+ * solver's current state (the work already enqueued on its stream is waited for); the call synchronises the stream
+ * before it returns.  It calls no cudaMalloc, cudaFree, or any other routine that allocates device memory.
+ *
+ * The limit.  The staging array holds DG_NOALLOC_MAX_VALUES doubles (4 MiB).  It is a static __device__ array of the
+ * library image, so every GPU on which the process uses the library carries these 4 MiB from the moment the library's
+ * device code is loaded there until the process exits, whether this call is used or not.  A solver with
+ * T*J*3*Nfp + E*J*J*2*(N+1) > DG_NOALLOC_MAX_VALUES gets DG_ENOMEM with a message that states both numbers, and
+ * nothing is launched (configs[0] needs 3,648 values, configs[1] 153,600; use dg_get_fields above that).
+ *
+ * First call on a device.  The library looks up the array's device address once per device (cudaGetSymbolAddress,
+ * with that device current) the first time the call is made for a solver on it.  Make that first call before any
+ * stream capture begins in the process.
+ *
+ * Sharing.  All solvers of the process on one device stage through the same array, and it keeps whatever the last
+ * call left in it.  Nothing needs clearing: each call overwrites exactly the values it then copies out and reads no
+ * other.  Two calls in flight at once on one GPU would overwrite each other's staging data, so the library holds a
+ * process-wide lock from the launch to the end of the copy-out; calls from several host threads therefore run one
+ * after the other, and the caller must not defeat this from outside (e.g. by sharing one solver between threads). */
+#define DG_NOALLOC_MAX_VALUES (1u << 19)
+int dg_get_aux_fields_noalloc(dg_solver* s, double* face_aux, double* edge_aux);
+
 const char* dg_last_error(void);
 /* Waits for the solver's stream, then frees what the library owns (never the caller's workspace). */
 void dg_destroy(dg_solver* s);

@@ -41,7 +41,8 @@ class _DeviceView(C.Structure):
 
 EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_set_source", "dg_step",
            "dg_get_fields", "dg_get_face_map", "dg_get_edge_map", "dg_reference_element", "dg_mesh_counts",
-           "dg_profile_step", "dg_last_step_kernel_ms", "dg_get_device_ptrs", "dg_last_error", "dg_destroy"]
+           "dg_profile_step", "dg_last_step_kernel_ms", "dg_get_device_ptrs", "dg_get_aux_fields_noalloc", "dg_last_error",
+           "dg_destroy"]
 
 
 def lib() -> C.CDLL:
@@ -192,6 +193,21 @@ class Solver:
         ea = np.zeros((self.E, self.J * self.J, 2, self.N + 1)) if aux else None
         _check(lib().dg_get_fields(self._h, _dp(q[0]), _dp(q[1]), _dp(q[2]), _dp(q[3]), _dp(fa), _dp(ea)))
         return q, fa, ea
+
+    NOALLOC_MAX_VALUES = 1 << 19                              # DG_NOALLOC_MAX_VALUES of include/dg_habc.h
+
+    def get_aux_fields_noalloc(self):
+        """dg_get_aux_fields_noalloc: (face_aux, edge_aux) exactly as get_fields() returns them, but staged on the GPU
+        through a fixed 4 MiB array built into libdg_habc.so instead of the solver's workspace, so the call never asks
+        for device memory.  It is meant for hosts that cannot allocate when they want the data -- all device memory
+        already given to another pool, another thread in a global-mode stream capture, a loop that cannot afford
+        cudaMalloc's device-wide synchronisation.  Solvers with more than NOALLOC_MAX_VALUES auxiliary values
+        (T*J*3*Nfp + E*J*J*2*(N+1)) raise DgError [-4].  The first call on a device looks up the array's address and
+        should come before any stream capture; calls are serialised inside the library because they share the array."""
+        fa = np.zeros((self.T, self.J, 3, self.Nfp))
+        ea = np.zeros((self.E, self.J * self.J, 2, self.N + 1))
+        _check(lib().dg_get_aux_fields_noalloc(self._h, _dp(fa), _dp(ea)))
+        return fa, ea
 
     def device_view(self):
         """dg_get_device_ptrs: raw device addresses of the current state in the library's layout (q [K][Np][4], face

@@ -1157,3 +1157,72 @@ int dg_profile_step(dg_solver* s, double* ms) {
 }
 
 }  // extern "C"
+
+// ======================================================================================= allocation-free read-back
+// dg_get_aux_fields_noalloc (include/dg_habc.h): k_export_aux staged through an array that is part of the library
+// image, for callers that have no way to obtain device memory (see the header for who they are).
+#include <mutex>
+
+// The staging area.  One instance per CUDA context that loads this module, DG_NOALLOC_MAX_VALUES doubles = 4 MiB, held
+// until the process exits.  In HOST code the name g_noalloc_stage is only a handle for the runtime's symbol calls: it
+// is not a device address and must never be handed to a kernel or to cudaMemcpy as a pointer.
+static __device__ __align__(256) double g_noalloc_stage[DG_NOALLOC_MAX_VALUES];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_lock;                                   // set-up table and the array itself (one call at a time)
+double* g_noalloc_addr[NOALLOC_MAX_DEVICES] = {};            // device address of g_noalloc_stage, per device ordinal
+
+// Device address of the staging array on `device`, which must be the current device.  Looked up on the first call
+// for that device and remembered; every later call is a table read.  Caller holds g_noalloc_lock.
+double* noalloc_stage_address(int device) {
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES)
+        throw std::runtime_error("EINVAL: dg_get_aux_fields_noalloc supports device ordinals 0..63");
+    if (!g_noalloc_addr[device]) {
+        double* ptr = nullptr;
+        cu(cudaGetSymbolAddress((void**)&ptr, g_noalloc_stage), "cudaGetSymbolAddress(staging array)");
+        if (!ptr) throw std::runtime_error("ECUDA: the staging array has no address on this device");
+        g_noalloc_addr[device] = ptr;
+    }
+    return g_noalloc_addr[device];
+}
+
+template <typename T>
+void export_aux_noalloc(dg_solver* s, Dev<T>& d, double* fa, double* ea) {
+    const size_t n2 = (size_t)d.Tn * d.J * 3 * d.Nfp, n1 = (size_t)d.E * d.J * d.J * 2 * d.N1, tot = n2 + n1;
+    if (tot > (size_t)DG_NOALLOC_MAX_VALUES)
+        throw std::runtime_error("ENOMEM: dg_get_aux_fields_noalloc: this solver has " + std::to_string(tot) +
+                                 " auxiliary values, the built-in staging array holds " +
+                                 std::to_string((size_t)DG_NOALLOC_MAX_VALUES) + "; use dg_get_fields");
+    if (tot == 0 || (!fa && !ea)) {                          // J = 0 or no HABC face: nothing to export
+        cu(cudaStreamSynchronize(s->stream), "sync");
+        return;
+    }
+    std::lock_guard<std::mutex> hold(g_noalloc_lock);        // until the copy-out is complete: the array is shared
+    double* stage = noalloc_stage_address(s->device);
+    // every value in [0, tot) is written here before the copies below read it; values beyond tot (left by a
+    // larger solver's call) are never read
+    k_export_aux<T><<<(unsigned)((tot + 255) / 256), 256, 0, s->stream>>>(d, s->cur, stage, stage + n2);
+    try {
+        cu(cudaGetLastError(), "export launch");
+        if (fa && n2) cu(cudaMemcpyAsync(fa, stage, sizeof(double) * n2, cudaMemcpyDeviceToHost, s->stream), "download");
+        if (ea && n1) cu(cudaMemcpyAsync(ea, stage + n2, sizeof(double) * n1, cudaMemcpyDeviceToHost, s->stream), "download");
+    } catch (...) {
+        cudaStreamSynchronize(s->stream);                    // the lock must outlive whatever was enqueued
+        throw;
+    }
+    cu(cudaStreamSynchronize(s->stream), "sync");
+}
+
+}  // namespace
+
+extern "C" int dg_get_aux_fields_noalloc(dg_solver* s, double* face_aux, double* edge_aux) {
+    try {
+        if (!s) throw std::runtime_error("EINVAL: NULL argument");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        if (s->precision == 64) export_aux_noalloc<double>(s, s->d64, face_aux, edge_aux);
+        else export_aux_noalloc<float>(s, s->d32, face_aux, edge_aux);
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
+}
