@@ -25,7 +25,8 @@ from workloads import CONFIGS, make_workload  # noqa: E402
 
 METRIC = "DG+HABC node-updates/sec"
 UNIT = "node-updates/s"
-# measured on this pool's B200 with paper_1610_05023_b200/csrc/ubench/peaks.cu (profiles/r01_peaks.md): DFMA 36.98,
+# measured on this pool's B200 with a DFMA / DMMA / FFMA microbenchmark (profiles/r01_peaks.md; the probe's source is a
+# working file, no longer tracked): DFMA 36.98,
 # DMMA 37.19 TFLOP/s (the same fp64 unit; the mixed DMMA+DFMA loop of that probe reaches 33.5), FFMA 71.2
 FP64_TFLOPS_MEASURED = 37.0
 FP32_TFLOPS_MEASURED = 71.2
@@ -116,7 +117,8 @@ def oracle_sample(workload: str, precision: int, budget_s: float = 20.0):
 
 
 def workload_config(name: str, w) -> dict:
-    """The part of `config` that names the workload; both arms (ours and --impl reference) print the same one."""
+    """The part of `config` that names the workload as it is really run: the GPU arm at full size, the --impl reference arm
+    on the bounded sample the oracle times (with `sample_of` naming the full configuration)."""
     Np = (w.N + 1) * (w.N + 2) * (w.N + 3) // 6
     return {"workload": name, "n_hex": w.n, "hex_grid": list(w.shape), "N": w.N, "J": w.J, "K": w.K, "nodes": w.K * Np}
 
@@ -146,7 +148,7 @@ def roofline(s, w, prec: int, prof: dict, workload: str, kernel_ms) -> dict:
     t_mem, t_alu = bytes_launch / (hbm_peak * 1e9), flops_launch / (alu_peak * 1e12)
     roof = dict(hbm if t_mem >= t_alu else alu)
     roof.update({"kernel": s.info["kernel_name"], "ms_per_launch": vol_ms,
-                 "ms_per_launch_source": "CUDA events around the kernel in the 5 stages of the last timed step, recorded in the replayed graph on the solver's stream",
+                 "ms_per_launch_source": "CUDA events around the kernel in the 5 stages of a step, recorded in the replayed graph on the solver's stream, in a short second timed run right after the headline one (which runs without the event nodes)",
                  "ms_per_launch_stages": [float(x) for x in kernel_ms], "ms_per_launch_profiled": prof["vol3d"] / 5.0,
                  "traffic": None, "traffic_source": None,
                  "roof_ms": 1e3 * max(t_mem, t_alu), "frac_of_slower_roof": max(t_mem, t_alu) / (vol_ms * 1e-3),
@@ -173,12 +175,14 @@ def run_reference(args):
         vals.append((v, step_s))
     vals = vals[args.warmup:]
     value = float(np.mean([v for v, _ in vals]))
-    w = make_workload(args.workload, n=args.n, N=args.N, J=args.J)
+    n_sample = min(CONFIGS[args.workload]["n"], 8)                    # what oracle_sample really times
+    w = make_workload(args.workload, n=n_sample)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([s for _, s in vals])),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": dict(workload_config(args.workload, w), parallelism="replicas only" if args.gpus > 1 else "single GPU",
-                           l2="state (q,res) exceeds L2 many times over; no flush needed"),
+            "config": dict(workload_config(args.workload, w), sample_of=args.workload,
+                           note="the numpy oracle times a bounded sample: this config's rule on the smaller grid named here, not the full-size mesh of the GPU arm",
+                           parallelism="host CPU, rank 0 only"),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "cores_available": avail, "kind": "oracle",
                              "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -194,8 +198,7 @@ def measure(args, w, prec: int, rep, local: int) -> dict:
 
     world = rep.world
     t_setup = time.perf_counter()
-    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, kernel=args.kernel, face_bc=w.face_bc,
-               time_kernels=True)
+    s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, kernel=args.kernel, face_bc=w.face_bc)
     x, y, z = s.get_nodes()
     cn = np.repeat(w.c[:, None], s.Np, axis=1)
     fields = [np.ascontiguousarray(f) for f in w.fields(x, y, z, cn, 1.0)]
@@ -219,7 +222,21 @@ def measure(args, w, prec: int, rep, local: int) -> dict:
     sampler.stop_flag = True
     ms = rep.max_over_ranks(ev0.elapsed_time(ev1))
     value = world * nodes * args.steps / (ms * 1e-3)
-    kernel_ms = s.last_step_kernel_ms()                            # the 3D kernel inside the last timed step
+
+    # ---- the dominant kernel inside a step: a second, short timed run with dg_options.time_kernels on (10 event-record
+    #      nodes per step in the replayed graph).  The headline above runs without them; both step times are reported.
+    s.set_time_kernels(True)
+    s.step(1)                                                      # capture + one untimed replay
+    nk = max(3, min(args.steps, 5))
+    evk0, evk1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(s.stream):
+        evk0.record(s.stream)
+        s.step(nk)
+        evk1.record(s.stream)
+    s.synchronize()
+    ms_step_events = evk0.elapsed_time(evk1) / nk
+    kernel_ms = s.last_step_kernel_ms()                            # the 3D kernel inside the last of those steps
+    s.set_time_kernels(False)
 
     # ---- per-kernel device time (outside the timed region): the dominant kernel's roofline
     prof = {k: 0.0 for k in ("vol3d", "face2d", "edge1d", "close_face", "close_edge", "close_corner")}
@@ -228,6 +245,9 @@ def measure(args, w, prec: int, rep, local: int) -> dict:
         for k, v in s.profile_step().items():
             prof[k] += v / nprof
     roof = roofline(s, w, prec, prof, args.workload, kernel_ms)
+    roof["ms_per_step_with_kernel_events"] = ms_step_events
+    roof["kernel_share_of_step"] = 5.0 * float(np.mean(kernel_ms)) / ms_step_events      # from the in-step events
+    roof["kernel_share_of_step_profiled"] = prof["vol3d"] / max(sum(prof.values()), 1e-12)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the four fp64 fields, the steps, D2H of
     #      the four fields, all inside the timed region

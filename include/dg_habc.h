@@ -89,7 +89,9 @@ typedef struct {
     double dt;
     uint64_t device_bytes;     /* device memory held by the solver */
     int32_t kernel;            /* the 3D kernel in use (DG_KERNEL_*, never DG_KERNEL_AUTO) */
-    char kernel_name[44];      /* its name as a profiler lists it, e.g. "k_vol3d_ws<5>" */
+    char kernel_name[44];      /* a short label "<kernel><N>", e.g. "k_vol3d_ws<5>": the kernel's template name and the degree.
+                                  A profiler prints the full instantiation (k_vol3d_mmag<6,2,8>, k_vol3d<double,5,4,4,true>),
+                                  of which this is a prefix up to the first template argument */
 } dg_info;
 
 /* Device bytes dg_create needs for this problem (lets the caller allocate the workspace, e.g. with torch). */
@@ -155,6 +157,11 @@ int dg_profile_step(dg_solver* s, double* ms);
  * the CUDA graph.  Synchronises the stream.  ms: [5], host. */
 int dg_last_step_kernel_ms(dg_solver* s, double* ms);
 
+/* Switch dg_options.time_kernels on or off on an existing solver (so that a benchmark can time its headline steps
+ * without the event nodes and read the per-stage kernel times from a few further steps with them).  Synchronises the
+ * stream and drops the captured step; the next dg_step captures it again.  The state is untouched. */
+int dg_set_time_kernels(dg_solver* s, int on);
+
 /* Raw device pointers of the current state, in the library's own layout (optional, lets a caller read
  * traces or fields on the device without the fp64 host round trip of dg_get_fields).  The pointers stay owned by the
  * library, are valid until dg_destroy, and hold the state reached by the work already enqueued on the solver's stream
@@ -208,7 +215,8 @@ int dg_get_device_ptrs(const dg_solver* s, dg_device_view* out);
 int dg_get_aux_fields_noalloc(dg_solver* s, double* face_aux, double* edge_aux);
 
 const char* dg_last_error(void);
-/* Waits for the solver's stream, then frees what the library owns (never the caller's workspace). */
+/* Waits for the solver's stream, then frees what the library owns (never the caller's workspace).  The stream given in
+ * dg_options must still exist; the caller's current device is restored and no CUDA error state is left behind. */
 void dg_destroy(dg_solver* s);
 
 #ifdef __cplusplus

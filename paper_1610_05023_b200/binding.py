@@ -41,7 +41,7 @@ class _DeviceView(C.Structure):
 
 EXPORTS = ["dg_workspace_bytes", "dg_create", "dg_get_info", "dg_get_nodes", "dg_set_initial", "dg_set_source", "dg_step",
            "dg_get_fields", "dg_get_face_map", "dg_get_edge_map", "dg_reference_element", "dg_mesh_counts",
-           "dg_profile_step", "dg_last_step_kernel_ms", "dg_get_device_ptrs", "dg_get_aux_fields_noalloc", "dg_last_error",
+           "dg_profile_step", "dg_last_step_kernel_ms", "dg_set_time_kernels", "dg_get_device_ptrs", "dg_get_aux_fields_noalloc", "dg_last_error",
            "dg_destroy"]
 
 
@@ -116,9 +116,11 @@ class Solver:
 
     def __init__(self, verts, tets, N: int, J: int, c, rho, precision: int = 64, cfl: float = 1.0,
                  dt: float = 0.0, device: int = 0, use_graph: bool = True, torch_workspace: bool = True,
-                 kernel: int = 0, face_bc=None, time_kernels: bool = False):
+                 kernel: int = 0, face_bc=None, time_kernels: bool = False, default_stream: bool = False):
         """face_bc: None (HABC everywhere) or {(axis, sign): "habc" | "dirichlet" | "rigid"} for some of the six domain
-        faces (axis 0..2, sign -1/+1) -- dg_options.face_bc."""
+        faces (axis 0..2, sign -1/+1) -- dg_options.face_bc.  torch_workspace = False: dg_options.workspace_dev = NULL,
+        the library allocates with cudaMalloc.  default_stream = True: dg_options.stream = NULL, the legacy default
+        stream (plain launches, no CUDA graph)."""
         import torch                                          # device memory + stream only
         if not torch.cuda.is_available():
             raise DgError("no CUDA device: the DG+HABC path has no CPU fallback")
@@ -135,9 +137,9 @@ class Solver:
         self._torch = torch
         torch.cuda.set_device(device)
         # a dedicated (capturable) torch stream: the solver's kernels and CUDA graph run on it
-        self._stream = torch.cuda.Stream(device=device)
+        self._stream = torch.cuda.default_stream(device) if default_stream else torch.cuda.Stream(device=device)
         self.stream = self._stream
-        opt.stream = self._stream.cuda_stream
+        opt.stream = None if default_stream else self._stream.cuda_stream
         self._ws = None
         if torch_workspace:
             nbytes = C.c_uint64(0)
@@ -236,6 +238,10 @@ class Solver:
         ms = np.zeros(5)
         _check(lib().dg_last_step_kernel_ms(self._h, _dp(ms)))
         return ms
+
+    def set_time_kernels(self, on: bool):
+        """dg_set_time_kernels: switch the per-stage kernel events of dg_options.time_kernels on or off."""
+        _check(lib().dg_set_time_kernels(self._h, int(bool(on))))
 
     def profile_step(self):
         ms = np.zeros(6)

@@ -422,10 +422,11 @@ void run_vol3d(dg_solver* s, Kern kern, int nthreads, size_t smem, int elems_per
                bool configure, Args... args) {
     if (configure) {
         cu(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "smem attr");
-        int per_sm = 1, sms = 0;
-        if (!one_per_sm) cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, nthreads, smem), "occupancy");
+        int per_sm = 0, sms = 0;
+        cu(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, nthreads, smem), "occupancy");
         cu(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device), "sm count");
-        if (per_sm < 1) throw std::runtime_error("ECUDA: the 3D kernel does not fit on an SM");
+        if (per_sm < 1) throw std::runtime_error("ECUDA: the 3D kernel does not fit on an SM");   // caught at dg_create
+        if (one_per_sm) per_sm = 1;
         const int nbatch = (K + elems_per_batch - 1) / elems_per_batch;
         s->grid3 = std::max(1, std::min(nbatch, per_sm * sms));
         s->smem3 = smem;
@@ -655,8 +656,12 @@ void run_step_plain(dg_solver* s, Dev<T>& d) {
 template <typename T>
 void run_steps(dg_solver* s, Dev<T>& d, int nsteps) {
     if (!s->use_graph) {
-        for (int i = 0; i < nsteps; ++i) { s->last_par = s->cur; run_step_plain<T>(s, d); }
-        cu(cudaGetLastError(), "kernel launch");
+        for (int i = 0; i < nsteps; ++i) {
+            s->last_par = s->cur;
+            run_step_plain<T>(s, d);
+            cu(cudaGetLastError(), "kernel launch");
+            s->t_host += s->dt;        // the host clock follows the steps that were really enqueued
+        }
         return;
     }
     for (int i = 0; i < nsteps; ++i) {
@@ -683,6 +688,7 @@ void run_steps(dg_solver* s, Dev<T>& d, int nsteps) {
         cu(cudaGraphLaunch(s->graph[par], s->stream), "graph launch");
         s->last_par = par;
         s->cur = par ^ 1;              // five stages flip the parity once
+        s->t_host += s->dt;
     }
 }
 
@@ -945,11 +951,16 @@ int dg_create(const dg_mesh* mesh, int N, int J, const double* c, const double* 
 
 void dg_destroy(dg_solver* s) {
     if (!s) return;
-    cudaSetDevice(s->device);
-    cudaStreamSynchronize(s->stream);      // dg_step is asynchronous: nothing may still be writing the workspace
-    for (int i = 0; i < 2; ++i) if (s->graph[i]) cudaGraphExecDestroy(s->graph[i]);
-    for (auto& par : s->evk) for (auto& st : par) for (auto& e : st) if (e) cudaEventDestroy(e);
-    if (s->own_ws && s->ws) cudaFree(s->ws);
+    int prev = -1;
+    cudaGetDevice(&prev);                  // the caller's current device is left as it was
+    if (cudaSetDevice(s->device) == cudaSuccess) {
+        cudaStreamSynchronize(s->stream);  // dg_step is asynchronous: nothing may still be writing the workspace
+        for (int i = 0; i < 2; ++i) if (s->graph[i]) cudaGraphExecDestroy(s->graph[i]);
+        for (auto& par : s->evk) for (auto& st : par) for (auto& e : st) if (e) cudaEventDestroy(e);
+        if (s->own_ws && s->ws) cudaFree(s->ws);
+    }
+    if (prev >= 0) cudaSetDevice(prev);
+    cudaGetLastError();                    // the return codes above are ignored on purpose: leave no stale error behind
     delete s;
 }
 
@@ -1054,7 +1065,6 @@ int dg_step(dg_solver* s, int nsteps) {
         cu(cudaSetDevice(s->device), "cudaSetDevice");
         if (s->precision == 64) run_steps<double>(s, s->d64, nsteps);
         else run_steps<float>(s, s->d32, nsteps);
-        for (int i = 0; i < nsteps; ++i) s->t_host += s->dt;
         return DG_OK;
     } catch (const std::exception& e) { return err_from_exception(e); }
 }
@@ -1110,6 +1120,23 @@ int dg_get_edge_map(const dg_solver* s, int32_t* axis, int32_t* normal_axes, int
                 }
     }
     return DG_OK;
+}
+
+int dg_set_time_kernels(dg_solver* s, int on) {
+    try {
+        if (!s) throw std::runtime_error("EINVAL: NULL argument");
+        cu(cudaSetDevice(s->device), "cudaSetDevice");
+        if ((on != 0) == s->time_kernels) return DG_OK;
+        cu(cudaStreamSynchronize(s->stream), "sync");
+        if (on)
+            for (auto& par : s->evk) for (auto& st : par) for (auto& e : st)
+                if (!e) cu(cudaEventCreate(&e), "event create");
+        s->time_kernels = on != 0;
+        s->last_par = -1;                          // no step has been timed under the new setting yet
+        for (int i = 0; i < 2; ++i)                 // the captured step has (or lacks) the event nodes: capture again
+            if (s->graph[i]) { cudaGraphExecDestroy(s->graph[i]); s->graph[i] = nullptr; }
+        return DG_OK;
+    } catch (const std::exception& e) { return err_from_exception(e); }
 }
 
 int dg_last_step_kernel_ms(dg_solver* s, double* ms) {

@@ -60,6 +60,7 @@ struct WsCfg {
     static constexpr int oBar = oN + NS * Nfn * EB * 4;  // full[NS], empty[NS], ready[2], opfree[2]
     static constexpr int oEnd = oBar + 2 * NS + 4;
     static constexpr size_t smem_bytes = sizeof(double) * oEnd + sizeof(int) * (33 * Nfp + Nfn) + 32;
+    static_assert(smem_bytes <= 227 * 1024, "shared memory");
     static constexpr uint32_t tx_bytes = 2 * EB * Np * 32 + EB * GX3 * 8;
     static constexpr int NJ = (Nfp + 3) / 4;           // face nodes per PREP thread (j = pw + 4 r)
     static constexpr int PITEM = (Nfn + 3) / 4;        // face nodes per LOADER lane
