@@ -111,14 +111,43 @@ def compare(lib, ora):
     return out
 
 
+def compare_same_order(got, ref):
+    """compare() for two results of the SAME code path family (library against library): cells, nodes and sets are in
+    the same order on both sides, so nothing is matched -- which keeps it affordable at 1.57 M cells -- but every field
+    and every auxiliary set is still judged on its own, against the norm of that field in `ref`.  Same keys as compare."""
+    qg, qr = got["q"], ref["q"]
+    out = {"p": rel_l2(qg[0], qr[0]), "norm_p": float(np.linalg.norm(qr[0]))}
+    for d, name in enumerate(("ux", "uy", "uz")):
+        out[name] = rel_l2(qg[1 + d], qr[1 + d])
+    out["u"] = max(out[k] for k in ("ux", "uy", "uz"))
+    out["norm_u"] = min(float(np.linalg.norm(qr[1 + d])) for d in range(3))
+    for grp, arr, names in (("face", "fa", ("p", "v1", "v2")), ("edge", "ea", ("p", "w"))):
+        a, b = got[arr], ref[arr]
+        if b.size == 0:
+            continue
+        nset = b.shape[1]
+        J = int(round(np.sqrt(nset)))
+        norms = {"p": [], "v": []}
+        for s_ in range(nset):
+            label = f"{s_}" if grp == "face" else f"{s_ // J},{s_ % J}"
+            for comp, name in enumerate(names):
+                out[f"{grp}_{name}[{label}]"] = rel_l2(a[:, s_, comp], b[:, s_, comp])
+                norms["p" if comp == 0 else "v"].append(float(np.linalg.norm(b[:, s_, comp])))
+        out[grp] = max(v for k, v in out.items() if k.startswith(grp + "_"))
+        out["norm_" + grp], out["norm_" + grp + "_vel"] = min(norms["p"]), min(norms["v"])
+    return out
+
+
 def worst(err, n=4):
     """the n largest per-field errors, for assertion messages"""
     items = [(k, v) for k, v in err.items() if not k.startswith("norm") and k not in ("u", "face", "edge")]
     return sorted(items, key=lambda kv: -kv[1])[:n]
 
 
-def check(err, tol, aux=True, floor_face=1e-3, floor_edge=1e-4, floor_vel=1e-6):
-    """tolerance on every field and every auxiliary set; pin P16 per set: each one carries data"""
+def check(err, tol, aux=True, floor_face=1e-3, floor_edge=1e-4, floor_vel=1e-4):
+    """tolerance on every field and every auxiliary set; pin P16 per set: each one carries data.  floor_vel: the
+    tangential velocities of the weakest auxiliary set measure 3e-2 (faces) / 4e-3 (edges) of ||p|| or more on the
+    workloads of the parity tests (oracle, 10 recipes); 1e-4 is far above fp32 round-off and well below those."""
     for k in ["p", "u"] + (["face", "edge"] if aux else []):
         assert err[k] <= tol, (k, err[k], worst(err))
     assert err["norm_p"] > 0
