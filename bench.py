@@ -48,6 +48,73 @@ def algorithmic_flops_per_element(N: int) -> float:
     return Np * (12 * Np + 24 + 8 * Nfp + 40) + 4 * Nfp * 14
 
 
+def habc_work_per_launch(N: int, J: int, T: int, E: int, C: int, precision: int) -> dict:
+    """DESIGN.md §7, HABC levels: algorithmic (bytes, flops) of ONE launch (one LSRK stage) of each auxiliary kernel.
+    Counts follow the arrays each kernel must touch: state and residual in and out, the closure sums, the neighbour /
+    parent traces, the per-cell records and tables; the small inverse matrices are counted once per launch."""
+    sz, Nfp, N1 = precision // 8, (N + 1) * (N + 2) // 2, N + 1
+    return {
+        "face2d": (T * (J * (12 * Nfp + 9 * N1) * sz + (Nfp + 3 * N1 + 23) * sz + 4 * (3 + 3 * N1)),
+                   T * J * (Nfp * (8 * Nfp + 6 * N1 + 30) + 3 * N1 * 14)),
+        "edge1d": (E * (J * J * (8 * N1 + 6) * sz + (2 * J * N1 + 8) * sz + 8),
+                   E * J * J * (N1 * (4 * N1 + 16) + 28)),
+        "close_face": (T * (Nfp * (J + 10) * sz + 16), T * Nfp * (2 * J + 12)),
+        "close_edge": (E * N1 * (J * J + 10 * J) * sz + 8 * J * J * sz, E * N1 * (14 * J * J + 12 * J)),
+        "close_corner": (C * 9 * J * J * sz + 9 * J ** 4 * sz, C * (18 * J ** 4 + 12 * J * J)),
+    }
+
+
+def sweep(local: int, hbm_peak: float) -> dict:
+    """BASELINE.json configs[3]: the 82,944-tet mesh at J = 4, N = 1..8, both precisions, per kernel: device time per
+    launch, algorithmic GB/s and TFLOP/s, fraction of the slower roof.  The 3D kernel is timed inside a replayed step
+    (dg_options.time_kernels), the auxiliary kernels by dg_profile_step (a host sync per launch, outside any timed
+    region)."""
+    import torch
+    from paper_1610_05023_b200 import Solver
+    cells = []
+    sampler = ClockSampler(local)
+    sampler.start()
+    for N in range(1, 9):
+        w = make_workload("cfg4", N=N, J=4)
+        for prec in (64, 32):
+            s = Solver(w.verts, w.tets, w.N, w.J, w.c, w.rho, precision=prec, device=local, time_kernels=True)
+            x, y, z = s.get_nodes()
+            cn = np.repeat(w.c[:, None], s.Np, axis=1)
+            s.set_initial(*w.fields(x, y, z, cn, 1.0))
+            s.step(3)
+            nst = 5
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(s.stream):
+                e0.record(s.stream)
+                s.step(nst)
+                e1.record(s.stream)
+            s.synchronize()
+            ms_step = e0.elapsed_time(e1) / nst
+            k3 = float(np.mean(s.last_step_kernel_ms()))
+            prof = s.profile_step()
+            alu_peak = FP64_TFLOPS_MEASURED if prec == 64 else FP32_TFLOPS_MEASURED
+
+            def row(name, ms, nbytes, nflops):
+                t_roof = max(nbytes / (hbm_peak * 1e9), nflops / (alu_peak * 1e12))
+                return {"kernel": name, "us": 1e3 * ms, "GBs": nbytes / (ms * 1e-3) / 1e9,
+                        "TFLOPs": nflops / (ms * 1e-3) / 1e12, "frac": t_roof / (ms * 1e-3)}
+            rows = [row(s.info["kernel_name"], k3, algorithmic_bytes_per_element(N, prec) * s.K,
+                        algorithmic_flops_per_element(N) * s.K)]
+            names = {"face2d": "k_face2d_mma" if prec == 64 and N <= 5 else "k_face2d", "edge1d": "k_edge1d",
+                     "close_face": "k_close_face", "close_edge": "k_close_edge", "close_corner": "k_close_corner"}
+            for key, (nbytes, nflops) in habc_work_per_launch(N, w.J, s.T, s.E, s.C, prec).items():
+                rows.append(row(names[key], prof[key] / 5.0, nbytes, nflops))
+            cells.append({"N": N, "J": w.J, "dtype": f"f{prec}", "K": s.K, "ms_per_step": ms_step,
+                          "node_updates_per_s": s.K * s.Np / (ms_step * 1e-3), "kernels": rows})
+            s.close()
+            del s
+    sampler.stop_flag = True
+    return {"workload": "cfg4 (82,944 tets), J = 4, N = 1..8", "steps_per_cell": 5, "warmup_per_cell": 3,
+            "units": {"us": "per launch", "GBs": "algorithmic bytes / time", "TFLOPs": "algorithmic flops / time",
+                      "frac": "slower-roof time / time (HBM peak below; ALU 37.0 / 71.2 TFLOP/s)"},
+            "hbm_peak_GBs": hbm_peak, "clocks": sampler.summary(), "cells": cells}
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons with NVML while the timed region runs."""
 
@@ -293,6 +360,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="dg_options.kernel (0 = the library's choice)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the run in the other precision")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the per-kernel degree sweep of configs[3]")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
     if args.impl == "reference":
@@ -324,6 +392,8 @@ def main():
         line["secondary"] = {"dtype": f"f{other}", "value": sec["value"], "unit": UNIT, "ms_per_step": sec["ms_per_step"],
                              "roofline": sec["roofline"], "e2e": sec["e2e"], "gpu_launches": sec["gpu_launches"],
                              "clocks": sec["clocks"], "run": sec["run"]}
+    if world == 1 and args.workload == "cfg5" and not args.no_sweep:
+        line["sweep"] = sweep(local, first["roofline"]["hbm"]["peak"])
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, desc, cores, _, avail = oracle_sample(args.workload, prec)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "cores_available": avail, "kind": "oracle",
