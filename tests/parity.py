@@ -144,10 +144,11 @@ def worst(err, n=4):
     return sorted(items, key=lambda kv: -kv[1])[:n]
 
 
-def check(err, tol, aux=True, floor_face=1e-3, floor_edge=1e-4, floor_vel=1e-4):
+def check(err, tol, aux=True, floor_face=1e-3, floor_edge=1e-4, floor_vel=1e-5):
     """tolerance on every field and every auxiliary set; pin P16 per set: each one carries data.  floor_vel: the
     tangential velocities of the weakest auxiliary set measure 3e-2 (faces) / 4e-3 (edges) of ||p|| or more on the
-    workloads of the parity tests (oracle, 10 recipes); 1e-4 is far above fp32 round-off and well below those."""
+    small workloads of the parity tests (oracle, 10 recipes) and 4.5e-5 (edges) over the whole 1.57 M-tet mesh of
+    configs[4], where ||p|| is taken over the full volume; 1e-5 is two orders above fp32 round-off and below all of them."""
     for k in ["p", "u"] + (["face", "edge"] if aux else []):
         assert err[k] <= tol, (k, err[k], worst(err))
     assert err["norm_p"] > 0
