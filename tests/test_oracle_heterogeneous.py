@@ -195,3 +195,36 @@ def test_boundary_levels_inherit_materials_as_reading_R9_states():
                  if np.abs(H.tri.x[t][:, a] - plane).max() < 1e-12 and has_points(H.tri.x[t], pts)]
         assert len(cands) == 1
         assert H.lin.c[e] == H.tri.c[cands[0]] and H.lin.rho[e] == H.tri.rho[cands[0]]
+
+
+def test_edge_outgoing_characteristic_uses_the_impedance_of_its_own_face():
+    """H5 (reading R9 inside the edge closure, eq (33)): the outgoing characteristic that a face's 2D
+    field sends across a domain edge is r^+ = (p + Z n.u)/2 with Z = rho c of THAT face's triangle.  With q = 0 and only
+    the tangential velocities of the triangle on side 0 of one line non-zero, every p_i00 vanishes, the edge system is
+    linear in r^+, and its solution must scale with that triangle's impedance and ignore the other side's.  (A closure
+    that takes Z from the triangle across the edge passes every other pin: found by mutation in round 3.)"""
+    from oracle.solver import OracleSolver
+    from workloads import cube_mesh
+    v, t = cube_mesh(2)
+    K, N, J = len(t), 2, 2
+    base = OracleSolver(v, t, N, J, np.ones(K), np.ones(K))
+    H = base.H
+    parent = H.tri_tetnode[:, 0] // H.tet.ref.Np
+    line = next(l for l in range(base.E) if parent[H.lin_tri[l, 0]] != parent[H.lin_tri[l, 1]])
+    rng = np.random.default_rng(3)
+    vel = rng.normal(size=(J, 2, H.tet.ref.Nfp))
+
+    def incoming(heavy_side):
+        rho = np.ones(K)
+        if heavy_side is not None:
+            rho[parent[H.lin_tri[line, heavy_side]]] = 3.0
+        o = OracleSolver(v, t, N, J, np.ones(K), rho)
+        assert np.array_equal(o.H.lin_tri, H.lin_tri)
+        q, fa, ea = np.zeros_like(o.q), np.zeros_like(o.fa), np.zeros_like(o.ea)
+        fa[:, 1:3, H.lin_tri[line, 0]] = vel
+        return o.closures((q, fa, ea))["rm_tri"]
+
+    r1, r_own, r_other = incoming(None), incoming(0), incoming(1)
+    assert np.linalg.norm(r1) > 1e-3
+    assert np.allclose(r_own, 3.0 * r1, rtol=1e-12, atol=1e-14)
+    assert np.allclose(r_other, r1, rtol=1e-12, atol=1e-14)
