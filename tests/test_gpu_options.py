@@ -128,3 +128,18 @@ def test_time_kernels_switched_on_an_existing_solver():
         s.close()
     for a, b in zip(*out):
         assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_random_per_cell_media_on_every_level(prec):
+    """c and rho drawn per TETRAHEDRON (not per layer or per hex as in the BASELINE recipes): neighbouring cells,
+    the two boundary triangles that meet at a domain edge, and consecutive lines then all differ in impedance, so the
+    heterogeneous flux of every level and the impedances inside the face / edge / corner closures (reading R9; oracle
+    pins H1-H5) are all exercised against the oracle."""
+    w = make_workload("cfg3", n=3, N=3, J=3, nsteps=25)
+    rng = np.random.default_rng(2025)
+    w.c = rng.uniform(1.0, 3.0, size=w.K)
+    w.rho = rng.uniform(0.5, 2.0, size=w.K)
+    lib, ora = parity.run_library(w, precision=prec), parity.run_oracle(w)
+    assert lib["dt"] == pytest.approx(ora["dt"], rel=1e-13)
+    parity.check(parity.compare(lib, ora), {64: 1e-11, 32: 1e-4}[prec])
